@@ -1,0 +1,111 @@
+/*
+ * rtcc.h -- C ABI of librtcc: the per-time-step hot path of the RT-EOM-CCSD cumulant Green's function
+ * method (arXiv:2301.04249; /root/reference/PAPER.md) on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (spin-explicit alpha-alpha / beta-beta / alpha-beta blocks, fp64, complex128
+ * amplitudes, real Cholesky vectors L^Q_pq with (pq|rs) = sum_Q L^Q_pq L^Q_rs):
+ *   R1_i^a   = <Phi_i^a  |(H_N e^{T1+T2})_C|Phi>     PAPER.md:76  Eq. 7
+ *   R2_ij^ab = <Phi_ij^ab|(H_N e^{T1+T2})_C|Phi>     PAPER.md:79  Eq. 8
+ *   E        = <Phi|(H_N e^{T})_C|Phi>               PAPER.md:58  Eq. 5 (integrand), :63 Eq. 6
+ *   i dt/dtau = -R  i.e. dt/dtau = +i R              PAPER.md:46  Eq. 2
+ *   t(tau+dt) = t(tau) + (i dt/2) [R(t(tau)) + R(t(tau+dt))]   PAPER.md:93 Eq. 9, fixed-point solved (:103)
+ *   C(tau)   = i int_0^tau E dtau'  by the trapezoid rule       PAPER.md:58 Eq. 5, :89
+ * with T1 = T2 = 0 and C = 0 at tau = 0.
+ *
+ * Conventions common to all calls
+ *   - Return value: 0 (RTCC_OK) or a negative error code; no exceptions, no aborts, nothing is printed.
+ *   - Array arguments are DEVICE pointers on the current CUDA device unless the context was created
+ *     with RTCC_HOST_PTRS, in which case every array argument of every call is a HOST pointer and the
+ *     library performs the copies (on its stream, synchronously).
+ *   - Complex arrays are interleaved (re, im) doubles.
+ *   - Packed amplitude layout (t1, r1: n_t1 complex; t2, r2: n_t2 complex):
+ *       t1 = [ alpha (i,a) at i*v_alpha + a | beta (I,A) at I*v_beta + A ]
+ *       t2 = [ alpha-alpha packed | beta-beta packed | alpha-beta full ]
+ *       same-spin element (i<j, a<b) at pair(i,j)*P(v) + pair(a,b), pair(x,y) = y(y-1)/2 + x, P(n)=n(n-1)/2;
+ *       alpha-beta element (i,J,a,B) at ((i*o_beta + J)*v_alpha + a)*v_beta + B.
+ *   - The caller owns every buffer it passes; the context owns all internal state.
+ *   - A context is not thread-safe; all work is issued on the stream given at creation.
+ */
+#ifndef RTCC_H
+#define RTCC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rtcc_ctx rtcc_ctx;
+
+enum {
+    RTCC_OK = 0,
+    RTCC_EINVAL = -1,     /* null pointer, non-positive size, o_a+v_a != o_b+v_b, dt not finite, ... */
+    RTCC_ENOMEM = -2,     /* device or host allocation failed */
+    RTCC_ECUDA = -3,      /* a CUDA call failed; rtcc_last_cuda_error() has the cudaError_t value */
+    RTCC_ENOCONV = -4,    /* micro-iterations reached max_micro; propagation state NOT advanced */
+    RTCC_ENONFINITE = -5  /* NaN/Inf met in the amplitude update; propagation state NOT advanced */
+};
+
+enum { RTCC_HOST_PTRS = 1u };
+
+/* Create a context for one (N-1)-electron problem.
+ *   o_alpha, o_beta >= 0, v_alpha, v_beta >= 1, o_alpha+v_alpha == o_beta+v_beta =: n, n_chol >= 1.
+ *   L    [2][n_chol][n][n] real, alpha then beta, each spin in its own [occupied | virtual] orbital order,
+ *        symmetric in (p,q).
+ *   fock [2][n][n] real symmetric Fock matrix of the (N-1)-electron reference (need not be diagonal).
+ *   Both are copied.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * State after creation: T1 = T2 = 0, C = 0, tau = 0, R(T=0) evaluated. */
+int rtcc_create(rtcc_ctx** out, int o_alpha, int o_beta, int v_alpha, int v_beta, int n_chol,
+                const double* L, const double* fock, unsigned flags, void* cuda_stream);
+void rtcc_destroy(rtcc_ctx* ctx);
+
+/* n_t1, n_t2: complex element counts of the packed arrays; workspace_bytes: device memory held. */
+int rtcc_sizes(const rtcc_ctx* ctx, long long* n_t1, long long* n_t2, long long* workspace_bytes);
+
+/* Pure evaluation of Eqs. 7-8 at the given amplitudes; does not touch the propagation state.
+ * r1/r2 receive R1/R2 in the packed layout. */
+int rtcc_residual(rtcc_ctx* ctx, const double* t1, const double* t2, double* r1, double* r2);
+/* Value of E = <Phi|(H_N e^T)_C|Phi> (Re, Im) computed by the most recent rtcc_residual call. */
+int rtcc_residual_energy(const rtcc_ctx* ctx, double out[2]);
+
+/* Restart support: set amplitudes, time and cumulant, re-evaluate R and E there. c is a HOST pointer. */
+int rtcc_set_amplitudes(rtcc_ctx* ctx, const double* t1, const double* t2, double time, const double c[2]);
+int rtcc_get_amplitudes(const rtcc_ctx* ctx, double* t1, double* t2);
+
+/* Solver of the implicit Eq. 9.  mode 0: plain fixed point t(k+1) = B + (i dt/2) R(t(k));
+ * mode 1: orbital-energy-denominator preconditioned iteration with the same fixed point.
+ * Converged when max |t(k+1)-t(k)| over all packed elements < tol; fixed_micro > 0 performs exactly that many
+ * iterations instead.  Defaults: mode 0, tol 1e-4, max_micro 200, fixed_micro 0. */
+int rtcc_set_solver(rtcc_ctx* ctx, int mode, double tol, int max_micro, int fixed_micro);
+
+/* Advance tau -> tau + dt by Eq. 9 and update the cumulant by the trapezoid rule. */
+int rtcc_step(rtcc_ctx* ctx, double dt);
+/* out (HOST): Re C, Im C, Re E, Im E at the current time; E = -i dC/dtau. */
+int rtcc_cumulant(const rtcc_ctx* ctx, double out[4]);
+int rtcc_last_micro_iterations(const rtcc_ctx* ctx);
+double rtcc_time(const rtcc_ctx* ctx);
+
+/* Instrumentation: kernel launches and executed tensor-pipe flops since creation / since last reset. */
+int rtcc_counters(const rtcc_ctx* ctx, long long* launches, double* dmma_flops);
+int rtcc_reset_counters(rtcc_ctx* ctx);
+/* Device time (ms) and executed flops of the pp-ladder kernels of the most recent residual evaluation
+ * that ran with timing enabled (rtcc_set_timing(ctx, 1) brackets them with CUDA events). */
+int rtcc_set_timing(rtcc_ctx* ctx, int on);
+int rtcc_ladder_timing(const rtcc_ctx* ctx, double* ms, double* flops, double* model_flops);
+
+/* Measured FP64 tensor-pipe peak (TFLOP/s) of the current device: register-resident DMMA loop. */
+int rtcc_fp64_peak(double* tflops);
+
+/* Test hook: copy a named internal buffer (e.g. "Zsc", "Yab", "Mq") to a HOST array; returns the number
+ * of doubles the buffer holds (or a negative error), copying at most max_doubles. */
+long long rtcc_debug_buffer(const rtcc_ctx* ctx, const char* name, double* out, long long max_doubles);
+
+/* Test hook for the contraction primitive: C[M][N] = alpha * A[M][K] * B[K][N] + beta * C, all dense row-major
+ * HOST arrays; cplx != 0 treats A, B, C as planar complex ([2][rows][cols]). */
+int rtcc_debug_gemm(int M, int N, int K, const double* A, const double* B, double* C, double alpha, double beta, int cplx);
+
+int rtcc_last_cuda_error(const rtcc_ctx* ctx);
+const char* rtcc_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

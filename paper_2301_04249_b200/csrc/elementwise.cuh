@@ -1,0 +1,455 @@
+// elementwise.cuh -- bandwidth-bound kernels of the RT-EOM-CCSD hot path: spin-block unpacking of the
+// packed boundary amplitudes into the contraction layouts, assembly / antisymmetrisation of the
+// residual (PAPER.md:133 spin-explicit blocks), the Adams-Moulton update (Eq. 9) and the
+// deterministic reductions for the cumulant rate (Eqs. 5-6).
+//
+// Complex arrays inside the library are "row-planar": element (r, c) of a matrix with `cols` columns
+// has its real part at r*2*cols + c and its imaginary part at r*2*cols + cols + c, so every row is a
+// Re|Im-stacked real row (north_star: "stacking Re and Im").  Packed boundary arrays are interleaved.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace rtcc {
+
+struct Dims {
+    int o[2], v[2], n, NQ;
+    int n1a, n1b, n1;        // spin-conserving ov pairs: alpha (i,a) then beta
+    int nA, nB;              // spin-flip pairs: A = (i alpha, B beta), B = (I beta, a alpha)
+    int po[2], pv[2];        // P(o), P(v)
+    int oo;                  // o_alpha * o_beta
+    long long off_t1[2];     // offsets (complex elements) into packed t1
+    long long off_t2[3];     // aa, bb, ab offsets into packed t2
+    long long n_t1, n_t2;
+};
+
+__host__ __device__ inline long long pair_index(int x, int y) { return (long long)y * (y - 1) / 2 + x; }
+
+struct c128 { double re, im; };
+
+// antisymmetric same-spin amplitude t_{im}^{ae} from the packed block
+__device__ __forceinline__ c128 ss_amp(const double* t2p, long long off, int pv, int i, int m, int a, int e)
+{
+    c128 z = {0.0, 0.0};
+    if (i == m || a == e) return z;
+    double s = 1.0;
+    if (i > m) { int t = i; i = m; m = t; s = -s; }
+    if (a > e) { int t = a; a = e; e = t; s = -s; }
+    long long k = off + pair_index(i, m) * pv + pair_index(a, e);
+    z.re = s * t2p[2 * k]; z.im = s * t2p[2 * k + 1];
+    return z;
+}
+__device__ __forceinline__ c128 ab_amp(const double* t2p, const Dims& d, int i, int J, int a, int B)
+{
+    long long k = d.off_t2[2] + (((long long)i * d.o[1] + J) * d.v[0] + a) * d.v[1] + B;
+    c128 z = {t2p[2 * k], t2p[2 * k + 1]};
+    return z;
+}
+
+// t1 packed -> planar t1r[pl][x], x in sc pair order (alpha (i,a) then beta)
+__global__ void k_unpack_t1(Dims d, const double* __restrict__ t1p, double* __restrict__ t1r)
+{
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < d.n1; x += (long long)gridDim.x * blockDim.x) {
+        t1r[x] = t1p[2 * x];
+        t1r[d.n1 + x] = t1p[2 * x + 1];
+    }
+}
+
+// Tsc[(s,i,a)][pl][(s',m,e)] = t_{im}^{ae}
+__global__ void k_build_Tsc(Dims d, const double* __restrict__ t2p, double* __restrict__ Tsc)
+{
+    const long long tot = (long long)d.n1 * d.n1;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        int r = (int)(x / d.n1), c = (int)(x - (long long)r * d.n1);
+        int sr = r >= d.n1a, sc = c >= d.n1a;
+        int rr = sr ? r - d.n1a : r, cc = sc ? c - d.n1a : c;
+        int i = rr / d.v[sr], a = rr - i * d.v[sr];
+        int m = cc / d.v[sc], e = cc - m * d.v[sc];
+        c128 z;
+        if (sr == sc) z = ss_amp(t2p, d.off_t2[sr], d.pv[sr], i, m, a, e);
+        else if (sr == 0) z = ab_amp(t2p, d, i, m, a, e);
+        else z = ab_amp(t2p, d, m, i, e, a);
+        Tsc[(long long)r * 2 * d.n1 + c] = z.re;
+        Tsc[(long long)r * 2 * d.n1 + d.n1 + c] = z.im;
+    }
+}
+
+// T_AB[(i,B)][pl][(M,e)] = -tab[i,M,e,B]
+__global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __restrict__ TAB)
+{
+    const long long tot = (long long)d.nA * d.nB;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        int r = (int)(x / d.nB), c = (int)(x - (long long)r * d.nB);
+        int i = r / d.v[1], B = r - i * d.v[1];
+        int M = c / d.v[0], e = c - M * d.v[0];
+        c128 z = ab_amp(t2p, d, i, M, e, B);
+        TAB[(long long)r * 2 * d.nB + c] = -z.re;
+        TAB[(long long)r * 2 * d.nB + d.nB + c] = -z.im;
+    }
+}
+
+// X_ab[(e,F)][pl][(i,J)] = tab[i,J,e,F];  tau_ab = X + t1a[i,e] t1b[J,F]
+__global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double* __restrict__ t1r,
+                            double* __restrict__ X, double* __restrict__ tau)
+{
+    const long long tot = (long long)d.v[0] * d.v[1] * d.oo;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        long long row = x / d.oo; int col = (int)(x - row * d.oo);
+        int e = (int)(row / d.v[1]), F = (int)(row - (long long)e * d.v[1]);
+        int i = col / d.o[1], J = col - i * d.o[1];
+        c128 z = ab_amp(t2p, d, i, J, e, F);
+        long long xa = (long long)i * d.v[0] + e, xb = d.n1a + (long long)J * d.v[1] + F;
+        double ar = t1r[xa], ai = t1r[d.n1 + xa], br = t1r[xb], bi = t1r[d.n1 + xb];
+        X[row * 2 * d.oo + col] = z.re;
+        X[row * 2 * d.oo + d.oo + col] = z.im;
+        tau[row * 2 * d.oo + col] = z.re + ar * br - ai * bi;
+        tau[row * 2 * d.oo + d.oo + col] = z.im + ar * bi + ai * br;
+    }
+}
+
+// X_ss[(e,f)][pl][(i<j)] = t_{ij}^{ef};  tau = X + t1[i,e] t1[j,f] - t1[i,f] t1[j,e]
+__global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const double* __restrict__ t1r,
+                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ tau)
+{
+    const int v = d.v[s], po = d.po[s];
+    const long long tot = (long long)v * v * po;
+    const long long o1 = s ? d.n1a : 0;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        long long row = x / po; int col = (int)(x - row * po);
+        int e = (int)(row / v), f = (int)(row - (long long)e * v);
+        int2 ij = opairs[col];
+        c128 z = ss_amp(t2p, d.off_t2[s], d.pv[s], ij.x, ij.y, e, f);
+        long long ie = o1 + (long long)ij.x * v + e, jf = o1 + (long long)ij.y * v + f;
+        long long iff = o1 + (long long)ij.x * v + f, je = o1 + (long long)ij.y * v + e;
+        double tr = t1r[ie] * t1r[jf] - t1r[d.n1 + ie] * t1r[d.n1 + jf] - (t1r[iff] * t1r[je] - t1r[d.n1 + iff] * t1r[d.n1 + je]);
+        double ti = t1r[ie] * t1r[d.n1 + jf] + t1r[d.n1 + ie] * t1r[jf] - (t1r[iff] * t1r[d.n1 + je] + t1r[d.n1 + iff] * t1r[je]);
+        X[row * 2 * po + col] = z.re;
+        X[row * 2 * po + po + col] = z.im;
+        tau[row * 2 * po + col] = z.re + tr;
+        tau[row * 2 * po + po + col] = z.im + ti;
+    }
+}
+
+// Mq[Q][pl][(s,i,a)] += Lt[s][pl][Q][o+a][i]      (N^Q_ia = L~^Q_ai + M^Q_ia)
+__global__ void k_add_Lvo(Dims d, const double* __restrict__ Lt0, const double* __restrict__ Lt1, double* __restrict__ Mq)
+{
+    const long long tot = (long long)d.NQ * 2 * d.n1;
+    const long long nn = (long long)d.n * d.n, plane = (long long)d.NQ * nn;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        long long Q = x / (2 * d.n1); int r = (int)(x - Q * 2 * d.n1);
+        int pl = r >= d.n1; int c = pl ? r - d.n1 : r;
+        int s = c >= d.n1a; int cc = s ? c - d.n1a : c;
+        int i = cc / d.v[s], a = cc - i * d.v[s];
+        const double* Lt = s ? Lt1 : Lt0;
+        Mq[x] += Lt[pl * plane + Q * nn + (long long)(d.o[s] + a) * d.n + i];
+    }
+}
+
+// W[(m,e)][pl][(j,b)] += -1/2 delta_mj Fvv[b][e] + 1/2 delta_be Foo[m][j]
+// (Fvv / Foo are the vv / oo blocks of the two dressed-Fock buffers; rows are (m of spin so, e of spin sv))
+__global__ void k_add_Fd(int om, int ve, int n, const double* __restrict__ Fo, int oo_, const double* __restrict__ Fv, int ov_,
+                         double* __restrict__ W, long long ldW, long long poff, long long roff, long long coff)
+{
+    // Fo: dressed Fock of the occupied index' spin (planar [2][n][n]), oo_ = its o; Fv likewise for the virtual index
+    const long long nn = (long long)n * n;
+    const long long tot1 = (long long)om * ve * ve, tot2 = (long long)om * om * ve;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot1 + tot2; x += (long long)gridDim.x * blockDim.x) {
+        for (int pl = 0; pl < 2; ++pl) {
+            if (x < tot1) {          // (m, e, b): j = m
+                int m = (int)(x / ((long long)ve * ve)); int r = (int)(x - (long long)m * ve * ve);
+                int e = r / ve, b = r - e * ve;
+                double f = Fv[pl * nn + (long long)(ov_ + b) * n + ov_ + e];
+                // b == e also gets the Foo[m][m] piece here so that each W element is touched by one thread only
+                double add = -0.5 * f;
+                if (b == e) add += 0.5 * Fo[pl * nn + (long long)m * n + m];
+                W[(roff + (long long)m * ve + e) * ldW + pl * poff + coff + (long long)m * ve + b] += add;
+            } else {                 // (m, j != m, e): b = e
+                long long y = x - tot1;
+                int m = (int)(y / ((long long)om * ve)); int r = (int)(y - (long long)m * om * ve);
+                int j = r / ve, e = r - j * ve;
+                if (j == m) continue;
+                double f = Fo[pl * nn + (long long)m * n + j];
+                W[(roff + (long long)m * ve + e) * ldW + pl * poff + coff + (long long)j * ve + e] += 0.5 * f;
+            }
+        }
+    }
+}
+
+// same-spin o^4 pieces: Wp[(m<n)][pl][(i<j)] = W4[(m,n)][(i,j)] - W4[(m,n)][(j,i)];  Yoop = rows (m,n) of Y
+__global__ void k_ss_prep(int o, int po, int n, const int2* __restrict__ opairs, const double* __restrict__ W4,
+                          const double* __restrict__ Y, double* __restrict__ Wp, double* __restrict__ Yoop)
+{
+    const long long tot = (long long)po * po;
+    const int o2 = o * o;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        int r = (int)(x / po), c = (int)(x - (long long)r * po);
+        int2 mn = opairs[r], ij = opairs[c];
+        long long row = (long long)(mn.x * o + mn.y) * 2 * o2;
+        for (int pl = 0; pl < 2; ++pl) {
+            Wp[(long long)r * 2 * po + pl * po + c] = W4[row + pl * o2 + ij.x * o + ij.y] - W4[row + pl * o2 + ij.y * o + ij.x];
+            Yoop[(long long)r * 2 * po + pl * po + c] = Y[((long long)mn.x * n + mn.y) * 2 * po + pl * po + c];
+        }
+    }
+}
+
+struct AsmArgs {
+    const double *Zsc, *ZAB, *ZBA, *Yab, *Yss[2], *Zv[2], *r1buf, *Ft[2];
+    const int2 *opairs[2], *vpairs[2];
+    double *r1p, *r2p;
+};
+
+// residual in the packed boundary layout (interleaved complex):
+//   r2 = P(ij)P(ab) Z + ladder pieces, r1 = r1buf + f~_ai
+__global__ void k_assemble(Dims d, AsmArgs A)
+{
+    const long long nss0 = (long long)d.po[0] * d.pv[0], nss1 = (long long)d.po[1] * d.pv[1];
+    const long long tot = d.n_t2 + d.n_t1;
+    const long long ld = 2LL * d.n1;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        double out[2];
+        if (x >= d.n_t2) {
+            long long k = x - d.n_t2;
+            int s = k >= d.n1a; int cc = (int)(s ? k - d.n1a : k);
+            int i = cc / d.v[s], a = cc - i * d.v[s];
+            const long long nn = (long long)d.n * d.n;
+            for (int pl = 0; pl < 2; ++pl)
+                out[pl] = A.r1buf[pl * (long long)d.n1 + k] + A.Ft[s][pl * nn + (long long)(d.o[s] + a) * d.n + i];
+            A.r1p[2 * k] = out[0]; A.r1p[2 * k + 1] = out[1];
+            continue;
+        }
+        if (x < nss0 + nss1) {
+            int s = x >= nss0; long long k = s ? x - nss0 : x;
+            int pij = (int)(k / d.pv[s]), pab = (int)(k - (long long)pij * d.pv[s]);
+            int2 ij = A.opairs[s][pij], ab = A.vpairs[s][pab];
+            const int v = d.v[s], po = d.po[s], o = d.o[s];
+            const long long off = s ? d.n1a : 0;
+            long long ia = off + ij.x * v + ab.x, jb = off + ij.y * v + ab.y, ja = off + ij.y * v + ab.x, ib = off + ij.x * v + ab.y;
+            for (int pl = 0; pl < 2; ++pl) {
+                long long p = pl * (long long)d.n1;
+                double z = A.Zsc[ia * ld + p + jb] - A.Zsc[ja * ld + p + ib] - A.Zsc[ib * ld + p + ja] + A.Zsc[jb * ld + p + ia];
+                z += A.Yss[s][((long long)(o + ab.x) * d.n + o + ab.y) * 2 * po + pl * po + pij];
+                z += -A.Zv[s][((long long)ab.x * v + ab.y) * 2 * po + pl * po + pij] + A.Zv[s][((long long)ab.y * v + ab.x) * 2 * po + pl * po + pij];
+                out[pl] = z;
+            }
+        } else {
+            long long k = x - nss0 - nss1;
+            int B = (int)(k % d.v[1]); k /= d.v[1];
+            int a = (int)(k % d.v[0]); k /= d.v[0];
+            int J = (int)(k % d.o[1]); int i = (int)(k / d.o[1]);
+            long long ia = (long long)i * d.v[0] + a, JB = d.n1a + (long long)J * d.v[1] + B;
+            long long iB = (long long)i * d.v[1] + B, Ja = (long long)J * d.v[0] + a;
+            for (int pl = 0; pl < 2; ++pl) {
+                double z = A.Zsc[ia * ld + pl * (long long)d.n1 + JB] + A.Zsc[JB * ld + pl * (long long)d.n1 + ia];
+                z -= A.ZAB[iB * 2 * d.nB + pl * (long long)d.nB + Ja];
+                z -= A.ZBA[Ja * 2 * d.nA + pl * (long long)d.nA + iB];
+                z += A.Yab[((long long)(d.o[0] + a) * d.n + d.o[1] + B) * 2 * d.oo + pl * d.oo + i * d.o[1] + J];
+                out[pl] = z;
+            }
+        }
+        A.r2p[2 * x] = out[0]; A.r2p[2 * x + 1] = out[1];
+    }
+}
+
+// ---------------------------------------------------------------- reductions (deterministic)
+constexpr int RED_BLOCKS = 296, RED_THREADS = 256;
+
+__device__ __forceinline__ double block_sum(double v, double* sh)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0) for (int i = 0; i < (int)(blockDim.x >> 5); ++i) r += sh[i];
+    return r;      // valid on thread 0
+}
+__device__ __forceinline__ double block_max(double v, double* sh)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x == 0) for (int i = 0; i < (int)(blockDim.x >> 5); ++i) r = fmax(r, sh[i]);
+    return r;
+}
+
+struct EnergyArgs {
+    const double* L[2]; const double* Lt[2]; const double* fock[2];   // bare vectors, dressed vectors (planar), bare Fock
+    const double* t1r; const double* Mq; const double* gam; double* partial;   // partial[RED_BLOCKS][2]
+};
+
+// E = sum f_ia t_i^a + 1/2 [ sum_Q,ia L_ia M_ia + sum_Q gamma_Q^2 - sum_s sum_Q,ij U_ji U_ij ],  U = L~_oo - L_oo
+// (Eq. 5 integrand PAPER.md:58).  Mq must still hold the bare M^Q (before k_add_Lvo).
+__global__ void __launch_bounds__(RED_THREADS) k_energy(Dims d, EnergyArgs A)
+{
+    __shared__ double sh[32];
+    double sr = 0.0, si = 0.0;
+    const long long nn = (long long)d.n * d.n, plane = (long long)d.NQ * nn;
+    const long long nT = d.n1, nM = (long long)d.NQ * d.n1, nG = d.NQ;
+    const long long nU0 = (long long)d.NQ * d.o[0] * d.o[0], nU1 = (long long)d.NQ * d.o[1] * d.o[1];
+    const long long tot = nT + nM + nG + nU0 + nU1;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        long long y = x;
+        if (y < nT) {
+            int s = y >= d.n1a; int cc = (int)(s ? y - d.n1a : y);
+            int i = cc / d.v[s], a = cc - i * d.v[s];
+            double f = A.fock[s][(long long)i * d.n + d.o[s] + a];
+            sr += f * A.t1r[y]; si += f * A.t1r[d.n1 + y];
+            continue;
+        }
+        y -= nT;
+        if (y < nM) {
+            long long Q = y / d.n1; int c = (int)(y - Q * d.n1);
+            int s = c >= d.n1a; int cc = s ? c - d.n1a : c;
+            int i = cc / d.v[s], a = cc - i * d.v[s];
+            double l = 0.5 * A.L[s][Q * nn + (long long)i * d.n + d.o[s] + a];
+            sr += l * A.Mq[Q * 2 * d.n1 + c]; si += l * A.Mq[Q * 2 * d.n1 + d.n1 + c];
+            continue;
+        }
+        y -= nM;
+        if (y < nG) {
+            double gr = A.gam[y], gi = A.gam[d.NQ + y];
+            sr += 0.5 * (gr * gr - gi * gi); si += gr * gi;
+            continue;
+        }
+        y -= nG;
+        int s = 0;
+        if (y >= nU0) { y -= nU0; s = 1; }
+        const int o = d.o[s];
+        long long Q = y / (o * o); int r = (int)(y - Q * o * o);
+        int i = r / o, j = r - i * o;
+        long long ij = Q * nn + (long long)i * d.n + j, ji = Q * nn + (long long)j * d.n + i;
+        double ur = A.Lt[s][ij] - A.L[s][ij], ui = A.Lt[s][plane + ij];
+        double wr = A.Lt[s][ji] - A.L[s][ji], wi = A.Lt[s][plane + ji];
+        sr -= 0.5 * (ur * wr - ui * wi); si -= 0.5 * (ur * wi + ui * wr);
+    }
+    double a = block_sum(sr, sh);
+    double b = block_sum(si, sh);
+    if (threadIdx.x == 0) { A.partial[2 * blockIdx.x] = a; A.partial[2 * blockIdx.x + 1] = b; }
+}
+
+__global__ void k_sum_partials(const double* __restrict__ partial, int nblocks, double* __restrict__ out2)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int i = 0; i < nblocks; ++i) { a += partial[2 * i]; b += partial[2 * i + 1]; }
+        out2[0] = a; out2[1] = b;
+    }
+}
+
+// y = a + (hr + i*hi) * r over n complex (interleaved) elements
+__global__ void k_caxpy(long long n, const double* __restrict__ a, const double* __restrict__ r, double hr, double hi,
+                        double* __restrict__ y)
+{
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n; x += (long long)gridDim.x * blockDim.x) {
+        double2 av = reinterpret_cast<const double2*>(a)[x], rv = reinterpret_cast<const double2*>(r)[x];
+        double2 o;
+        o.x = av.x + hr * rv.x - hi * rv.y;
+        o.y = av.y + hr * rv.y + hi * rv.x;
+        reinterpret_cast<double2*>(y)[x] = o;
+    }
+}
+
+// Adams-Moulton micro-iteration (Eq. 9):
+//   mode 0:  y = B + h R(x)                       h = i dt/2
+//   mode 1:  y = (B + h (R(x) - D x)) / (1 - h D) D = orbital-energy denominator (same fixed point)
+// writes y, and the block maxima of |y - x| (a non-finite value is reported as +inf).
+__global__ void __launch_bounds__(RED_THREADS) k_am_update(long long n, const double* __restrict__ Bv, const double* __restrict__ R,
+                                                           const double* __restrict__ xin, const double* __restrict__ Dn, int mode,
+                                                           double dt_half, double* __restrict__ y, double* __restrict__ bmax)
+{
+    __shared__ double sh[32];
+    double mx = 0.0;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n; x += (long long)gridDim.x * blockDim.x) {
+        double2 b = reinterpret_cast<const double2*>(Bv)[x], r = reinterpret_cast<const double2*>(R)[x];
+        double2 t = reinterpret_cast<const double2*>(xin)[x], o;
+        if (mode == 0) {
+            o.x = b.x - dt_half * r.y;
+            o.y = b.y + dt_half * r.x;
+        } else {
+            double D = Dn[x];
+            double gr = r.x - D * t.x, gi = r.y - D * t.y;          // R - D x
+            double nr = b.x - dt_half * gi, ni = b.y + dt_half * gr; // B + h (R - D x)
+            double c = dt_half * D;                                   // 1 - h D = 1 - i c
+            double den = 1.0 / (1.0 + c * c);
+            o.x = (nr - c * ni) * den;                                // (nr + i ni)(1 + i c)/(1+c^2)
+            o.y = (ni + c * nr) * den;
+        }
+        reinterpret_cast<double2*>(y)[x] = o;
+        double dx = o.x - t.x, dy = o.y - t.y;
+        double a = sqrt(dx * dx + dy * dy);
+        if (!(a == a) || isinf(a)) a = INFINITY;
+        mx = fmax(mx, a);
+    }
+    double m = block_max(mx, sh);
+    if (threadIdx.x == 0) bmax[blockIdx.x] = m;
+}
+
+__global__ void k_max_partials(const double* __restrict__ bmax, int n, double* __restrict__ out)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double m = 0.0;
+        for (int i = 0; i < n; ++i) m = fmax(m, bmax[i]);
+        out[0] = m;
+    }
+}
+
+// orbital-energy denominators of every packed element (t1 then t2): D = f_aa (+ f_bb) - f_ii (- f_jj)
+__global__ void k_build_Dn(Dims d, const double* __restrict__ f0, const double* __restrict__ f1,
+                           const int2* __restrict__ op0, const int2* __restrict__ op1,
+                           const int2* __restrict__ vp0, const int2* __restrict__ vp1, double* __restrict__ Dn)
+{
+    const long long nss0 = (long long)d.po[0] * d.pv[0], nss1 = (long long)d.po[1] * d.pv[1];
+    const long long tot = d.n_t1 + d.n_t2;
+    const int n = d.n;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        double D;
+        if (x < d.n_t1) {
+            int s = x >= d.n1a; int cc = (int)(s ? x - d.n1a : x);
+            int i = cc / d.v[s], a = cc - i * d.v[s];
+            const double* f = s ? f1 : f0;
+            D = f[(long long)(d.o[s] + a) * n + d.o[s] + a] - f[(long long)i * n + i];
+        } else {
+            long long k = x - d.n_t1;
+            if (k < nss0 + nss1) {
+                int s = k >= nss0; if (s) k -= nss0;
+                int pij = (int)(k / d.pv[s]), pab = (int)(k - (long long)pij * d.pv[s]);
+                int2 ij = (s ? op1 : op0)[pij], ab = (s ? vp1 : vp0)[pab];
+                const double* f = s ? f1 : f0; const int o = d.o[s];
+                D = f[(long long)(o + ab.x) * n + o + ab.x] + f[(long long)(o + ab.y) * n + o + ab.y]
+                  - f[(long long)ij.x * n + ij.x] - f[(long long)ij.y * n + ij.y];
+            } else {
+                k -= nss0 + nss1;
+                int B = (int)(k % d.v[1]); k /= d.v[1];
+                int a = (int)(k % d.v[0]); k /= d.v[0];
+                int J = (int)(k % d.o[1]); int i = (int)(k / d.o[1]);
+                D = f0[(long long)(d.o[0] + a) * n + d.o[0] + a] + f1[(long long)(d.o[1] + B) * n + d.o[1] + B]
+                  - f0[(long long)i * n + i] - f1[(long long)J * n + J];
+            }
+        }
+        Dn[x] = D;
+    }
+}
+
+// FP64 tensor-pipe peak probe: register-resident DMMA loop (denominator of the contraction roofline)
+__global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters, double seed)
+{
+    double acc[16][2], a[4], b[4];
+    for (int i = 0; i < 16; ++i) acc[i][0] = acc[i][1] = 0.0;
+    for (int i = 0; i < 4; ++i) { a[i] = seed * (threadIdx.x + i); b[i] = seed * (i + 1); }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                             : "+d"(acc[i * 4 + j][0]), "+d"(acc[i * 4 + j][1]) : "d"(a[i]), "d"(b[j]));
+    }
+    double s = 0.0;
+    for (int i = 0; i < 16; ++i) s += acc[i][0] + acc[i][1];
+    out[blockIdx.x * (long long)blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace rtcc

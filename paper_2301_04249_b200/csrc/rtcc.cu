@@ -1,0 +1,1053 @@
+// rtcc.cu -- context, residual pipeline, Adams-Moulton step driver and the C ABI of librtcc
+// (include/rtcc.h).  The working equations are the Cholesky / T1-dressed form of the spin-orbital
+// CCSD projections (Eqs. 7-8), restricted to the alpha-alpha / beta-beta / alpha-beta
+// blocks; DESIGN.md section 4 derives them.  Every contraction is a tcgemm launch
+// (tcgemm.cuh) except the particle-particle ladder (ladder.cuh); the rest is elementwise.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/rtcc.h"
+#include "elementwise.cuh"
+#include "ladder.cuh"
+#include "tcgemm.cuh"
+
+using namespace rtcc;
+
+struct rtcc_ctx {
+    Dims d{};
+    unsigned flags = 0;
+    cudaStream_t st = nullptr;
+    int num_sms = 148;
+    int cuda_err = 0;
+    std::vector<void*> allocs;
+    std::vector<std::pair<std::string, std::pair<double*, long long>>> named;
+    long long bytes = 0;
+
+    double *L[2]{}, *Lt[2]{}, *fockd[2]{}, *Fb[2]{}, *Ft[2]{}, *Kx[2]{}, *KxBA = nullptr;
+    double *t1r = nullptr, *Tsc = nullptr, *Wsc = nullptr, *Zsc = nullptr;
+    double *TAB = nullptr, *WBB = nullptr, *WAA = nullptr, *ZAB = nullptr, *ZBA = nullptr;
+    double *Mq = nullptr, *gam = nullptr, *r1buf = nullptr;
+    double *Xab = nullptr, *tauab = nullptr, *Yab = nullptr, *Wooab = nullptr;
+    double *Xss[2]{}, *tauss[2]{}, *Yss[2]{}, *W4[2]{}, *Wp[2]{}, *Yoop[2]{}, *Zv[2]{};
+    int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
+    int ntiles_ab = 0, ntiles_ss[2]{};
+    double* ws = nullptr; long long ws_cap = 0;
+    double *partial = nullptr, *bmax = nullptr, *scal = nullptr;   // scal: [0..1] E, [2] delta
+    double* h_scal = nullptr;                                      // pinned host mirror of scal
+    double *gx = nullptr, *gr = nullptr;                           // residual input / output (packed amp vectors)
+    double *t_cur = nullptr, *r_cur = nullptr, *Bv = nullptr, *Dn = nullptr;
+    double *io = nullptr;                                          // staging for host-pointer mode
+    long long namp = 0;                                            // n_t1 + n_t2 (complex)
+
+    // propagation state
+    double time = 0.0, C[2] = {0, 0}, E[2] = {0, 0}, E_res[2] = {0, 0};
+    int mode = 0, max_micro = 200, fixed_micro = 0, last_micro = 0;
+    double tol = 1e-4;
+
+    // instrumentation
+    long long launches = 0; double flops = 0.0;
+    long long res_launches = 0; double res_flops = 0.0;            // per residual evaluation
+    int timing = 0; cudaEvent_t ev[2]{}; double lad_ms = 0, lad_flops = 0, lad_model = 0;
+    cudaGraphExec_t graph = nullptr;
+    bool capturing = false;
+};
+
+namespace {
+
+#define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { c->cuda_err = (int)e_; return RTCC_ECUDA; } } while (0)
+
+template <class T> int dalloc(rtcc_ctx* c, T** p, long long count, const char* name = nullptr)
+{
+    if (count <= 0) count = 1;
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, (size_t)count * sizeof(T));
+    if (e != cudaSuccess) { c->cuda_err = (int)e; cudaGetLastError(); return RTCC_ENOMEM; }
+    c->allocs.push_back(q);
+    c->bytes += count * (long long)sizeof(T);
+    *p = (T*)q;
+    if (name) c->named.push_back({name, {(double*)q, count * (long long)sizeof(T) / 8}});
+    return 0;
+}
+
+TcGemm G0(int M, int N, int K)
+{
+    TcGemm g;
+    memset(&g, 0, sizeof(g));
+    g.M = M; g.N = N; g.K = K;
+    g.nb = 1; g.nsb = 1; g.alpha = 1.0; g.beta = 0.0; g.ksplit = 1;
+    for (int b = 0; b < TG_MAXB; ++b) { g.nphase[b] = 1; g.s0[b] = 1; g.s1[b] = 1; }
+    return g;
+}
+void setA(TcGemm& g, long long m_hi, long long m_lo, int Mlo, long long k_hi, long long k_lo, int Klo, int kfast)
+{ g.am_hi = m_hi; g.am_lo = m_lo; g.Mlo = Mlo; g.ak_hi = k_hi; g.ak_lo = k_lo; g.Klo = Klo; g.a_kfast = kfast; }
+void setB(TcGemm& g, long long k_hi, long long k_lo, long long n_hi, long long n_lo, int Nlo, int nfast)
+{ g.bk_hi = k_hi; g.bk_lo = k_lo; g.bn_hi = n_hi; g.bn_lo = n_lo; g.Nlo = Nlo; g.b_nfast = nfast; }
+void setC(TcGemm& g, long long m_hi, long long m_lo, long long n_hi, long long n_lo)
+{ g.cm_hi = m_hi; g.cm_lo = m_lo; g.cn_hi = n_hi; g.cn_lo = n_lo; }
+void ops_rr(TcGemm& g, const double* A, const double* B, double* C)
+{ g.nb = 1; g.A[0][0] = A; g.B[0][0] = B; g.C[0] = C; }
+void ops_rc(TcGemm& g, const double* A, const double* B, long long pB, double* C, long long pC)
+{ g.nb = 2; for (int b = 0; b < 2; ++b) { g.A[b][0] = A; g.B[b][0] = B + b * pB; g.C[b] = C + b * pC; } }
+void ops_cr(TcGemm& g, const double* A, long long pA, const double* B, double* C, long long pC)
+{ g.nb = 2; for (int b = 0; b < 2; ++b) { g.A[b][0] = A + b * pA; g.B[b][0] = B; g.C[b] = C + b * pC; } }
+void ops_cc(TcGemm& g, const double* A, long long pA, const double* B, long long pB, double* C, long long pC)
+{
+    g.nb = 2;
+    g.nphase[0] = g.nphase[1] = 2;
+    g.A[0][0] = A; g.B[0][0] = B; g.s0[0] = 1; g.A[0][1] = A + pA; g.B[0][1] = B + pB; g.s1[0] = -1; g.C[0] = C;
+    g.A[1][0] = A; g.B[1][0] = B + pB; g.s0[1] = 1; g.A[1][1] = A + pA; g.B[1][1] = B; g.s1[1] = 1; g.C[1] = C + pC;
+}
+void run(rtcc_ctx* c, TcGemm& g)
+{
+    g.ws = c->ws;
+    int n = tcgemm_launch(g, c->st, c->ws_cap, c->num_sms, &c->flops);
+    c->launches += n;
+}
+inline int nblk(long long n, int cap) { long long b = (n + 255) / 256; if (b < 1) b = 1; if (b > cap) b = cap; return (int)b; }
+#define EW(c, kern, n, ...) do { kern<<<nblk((n), (c)->num_sms * 16), 256, 0, (c)->st>>>(__VA_ARGS__); (c)->launches++; } while (0)
+
+}  // namespace
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// One evaluation of R1, R2 (Eqs. 7-8) and E (Eq. 5 integrand) at the packed amplitudes x -> r.
+// Only asynchronous work on c->st (capturable into a CUDA graph).
+// ---------------------------------------------------------------------------------------------
+int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
+{
+    const Dims& d = c->d;
+    const int n = d.n, NQ = d.NQ, n1 = d.n1;
+    const long long nn = (long long)n * n, plane = (long long)NQ * nn, ld1 = 2LL * n1;
+    const double* t1p = x;
+    const double* t2p = x + 2 * d.n_t1;
+    cudaStream_t st = c->st;
+
+    // ---- 1. unpack the packed spin blocks into the contraction layouts
+    EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
+    EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc);
+    EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB);
+    EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->tauab);
+    for (int s = 0; s < 2; ++s)
+        if (d.po[s] > 0)
+            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->tauss[s]);
+
+    // ---- 2. T1-dressed Cholesky vectors  L~^Q = (1-T) L^Q (1+T)
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        CK(cudaMemcpyAsync(c->Lt[s], c->L[s], plane * 8, cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemsetAsync(c->Lt[s] + plane, 0, plane * 8, st));
+        if (o == 0) continue;
+        {   // (L Y)[Q][p][i] += sum_e L[Q][p][o+e] t_i^e
+            TcGemm g = G0(NQ * n, o, v);
+            setA(g, 0, n, 0, 0, 1, 0, 1);
+            setB(g, 0, 1, 0, v, 0, 0);
+            setC(g, 0, n, 0, 1);
+            ops_rc(g, c->L[s] + o, c->t1r + off1, n1, c->Lt[s], plane);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // rows a: L~[Q][a][q] -= sum_m t_m^a (L Y)[Q][m][q]
+            TcGemm g = G0(v, NQ * n, o);
+            setA(g, 0, 1, 0, 0, v, 0, 0);
+            setB(g, 0, n, nn, 1, n, 1);
+            setC(g, 0, n, nn, 1);
+            ops_cc(g, c->t1r + off1, n1, c->Lt[s], plane, c->Lt[s] + (long long)o * n, plane);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 3. gamma^Q = sum_ie L^Q_ie t_i^e (both spins)
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        TcGemm g = G0(NQ, 1, o * v);
+        setA(g, 0, nn, 0, n, 1, v, 1);
+        setB(g, v, 1, 0, 0, 0, 0);
+        setC(g, 0, 1, 0, 0);
+        ops_rc(g, c->L[s] + o, c->t1r + off1, n1, c->gam, NQ);
+        g.beta = s ? 1.0 : 0.0;
+        run(c, g);
+    }
+
+    // ---- 4. M^Q_ia = sum_me L^Q_me t_im^ae over the spin-conserving pair space
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        TcGemm g = G0(NQ, 2 * n1, o * v);
+        setA(g, 0, nn, 0, n, 1, v, 1);
+        setB(g, v * ld1, ld1, 0, 1, 0, 1);
+        setC(g, 0, ld1, 0, 1);
+        ops_rr(g, c->L[s] + o, c->Tsc + off1 * ld1, c->Mq);
+        g.beta = s ? 1.0 : 0.0;
+        run(c, g);
+    }
+
+    // ---- 5. E (needs the bare M^Q)
+    {
+        EnergyArgs ea;
+        for (int s = 0; s < 2; ++s) { ea.L[s] = c->L[s]; ea.Lt[s] = c->Lt[s]; ea.fock[s] = c->fockd[s]; }
+        ea.t1r = c->t1r; ea.Mq = c->Mq; ea.gam = c->gam; ea.partial = c->partial;
+        k_energy<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d, ea);
+        k_sum_partials<<<1, 32, 0, st>>>(c->partial, RED_BLOCKS, c->scal);
+        c->launches += 2;
+    }
+
+    // ---- 6. dressed Fock  f~ = X (f + K_bare + sum_Q gamma^Q L^Q) Y - sum_Q,i L~^Q_pi L~^Q_iq
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        double* F = c->Ft[s];
+        CK(cudaMemcpyAsync(F, c->Fb[s], nn * 8, cudaMemcpyDeviceToDevice, st));
+        CK(cudaMemsetAsync(F + nn, 0, nn * 8, st));
+        {
+            TcGemm g = G0((int)nn, 1, NQ);
+            setA(g, 0, 1, 0, 0, nn, 0, 0);
+            setB(g, 0, 1, 0, 0, 0, 0);
+            setC(g, 0, 1, 0, 0);
+            ops_rc(g, c->L[s], c->gam, NQ, F, nn);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        if (o > 0) {
+            {
+                TcGemm g = G0(n, o, v);
+                setA(g, 0, n, 0, 0, 1, 0, 1);
+                setB(g, 0, 1, 0, v, 0, 0);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, F + o, nn, c->t1r + off1, n1, F, nn);
+                g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(v, n, o);
+                setA(g, 0, 1, 0, 0, v, 0, 0);
+                setB(g, 0, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, c->t1r + off1, n1, F, nn, F + (long long)o * n, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(n, n, NQ * o);
+                setA(g, 0, n, 0, nn, 1, o, 1);
+                setB(g, nn, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, c->Lt[s], plane, c->Lt[s], plane, F, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {   // F_ae = f~_ae - sum_Q,m L^Q_me M^Q_ma   (in place in the vv block)
+                TcGemm g = G0(v, v, NQ * o);
+                setA(g, 0, 1, 0, ld1, v, o, 0);
+                setB(g, nn, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cr(g, c->Mq + off1, n1, c->L[s] + o, F + (long long)o * n + o, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {   // F_mi = f~_mi + sum_Q,e L^Q_me M^Q_ie   (in place in the oo block)
+                TcGemm g = G0(o, o, NQ * v);
+                setA(g, 0, n, 0, nn, 1, v, 1);
+                setB(g, ld1, 1, 0, v, 0, 0);
+                setC(g, 0, n, 0, 1);
+                ops_rc(g, c->L[s] + o, c->Mq + off1, n1, F, nn);
+                g.beta = 1.0;
+                run(c, g);
+            }
+        }
+    }
+
+    // ---- 7. singles:  r1 = sum_me t_im^ae f~_me - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af   (+ f~_ai at assembly)
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        TcGemm g = G0(n1, 1, o * v);
+        setA(g, 0, ld1, 0, v, 1, v, 1);
+        setB(g, n, 1, 0, 0, 0, 0);
+        setC(g, 0, 1, 0, 0);
+        ops_cc(g, c->Tsc + off1, n1, c->Ft[s] + o, nn, c->r1buf, n1);
+        g.beta = s ? 1.0 : 0.0;
+        run(c, g);
+    }
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        if (o == 0) continue;
+        {
+            TcGemm g = G0(o, v, NQ * o);
+            setA(g, 0, 1, 0, nn, n, o, 0);
+            setB(g, ld1, v, 0, 1, 0, 1);
+            setC(g, 0, v, 0, 1);
+            ops_cc(g, c->Lt[s], plane, c->Mq + off1, n1, c->r1buf + off1, n1);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(o, v, NQ * v);
+            setA(g, 0, v, 0, ld1, 1, v, 1);
+            setB(g, nn, 1, 0, n, 0, 0);
+            setC(g, 0, v, 0, 1);
+            ops_cc(g, c->Mq + off1, n1, c->Lt[s] + (long long)o * n + o, plane, c->r1buf + off1, n1);
+            g.beta = 1.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 8. driver + Coulomb ring channel:  Zsc = 1/2 N^T N,  N^Q_ia = L~^Q_ai + M^Q_ia
+    EW(c, k_add_Lvo, (long long)NQ * 2 * n1, d, c->Lt[0], c->Lt[1], c->Mq);
+    {
+        TcGemm g = G0(n1, n1, NQ);
+        setA(g, 0, 1, 0, 0, ld1, 0, 0);
+        setB(g, 0, ld1, 0, 1, 0, 1);
+        setC(g, 0, ld1, 0, 1);
+        ops_cc(g, c->Mq, n1, c->Mq, n1, c->Zsc, n1);
+        g.alpha = 0.5;
+        run(c, g);
+    }
+
+    // ---- 9. exchange ring channel + F terms, spin-conserving sector:  Zsc -= T (Xd + 1/2 Kx T + Fd)
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s], n1s = o * v;
+        const long long off1 = s ? d.n1a : 0;
+        if (n1s == 0) continue;
+        {
+            TcGemm g = G0(n1s, 2 * n1, n1s);
+            setA(g, 0, n1s, 0, 0, 1, 0, 1);
+            setB(g, 0, ld1, 0, 1, 0, 1);
+            setC(g, 0, ld1, 0, 1);
+            ops_rr(g, c->Kx[s], c->Tsc + off1 * ld1, c->Wsc + off1 * ld1);
+            g.alpha = 0.5;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(o * o, v * v, NQ);
+            setA(g, n, 1, o, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, v, 1);
+            setC(g, (long long)v * ld1, v, 1, ld1);
+            ops_cc(g, c->Lt[s], plane, c->Lt[s] + (long long)o * n + o, plane, c->Wsc + off1 * ld1 + off1, n1);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1);
+    }
+    {
+        TcGemm g = G0(n1, n1, n1);
+        setA(g, 0, ld1, 0, 0, 1, 0, 1);
+        setB(g, 0, ld1, 0, 1, 0, 1);
+        setC(g, 0, ld1, 0, 1);
+        ops_cc(g, c->Tsc, n1, c->Wsc, n1, c->Zsc, n1);
+        g.alpha = -1.0; g.beta = 1.0;
+        run(c, g);
+    }
+
+    // ---- 10. spin-flip sector
+    if (d.nA > 0 && d.nB > 0) {
+        const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], nA = d.nA, nB = d.nB;
+        const long long lA = 2LL * nA, lB = 2LL * nB;
+        {
+            TcGemm g = G0(nB, 2 * nB, nA);
+            setA(g, 0, nA, 0, 0, 1, 0, 1);
+            setB(g, 0, lB, 0, 1, 0, 1);
+            setC(g, 0, lB, 0, 1);
+            ops_rr(g, c->KxBA, c->TAB, c->WBB);
+            g.alpha = 0.5;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(ob * ob, va * va, NQ);
+            setA(g, n, 1, ob, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, va, 1);
+            setC(g, va * lB, va, 1, lB);
+            ops_cc(g, c->Lt[1], plane, c->Lt[0] + (long long)oa * n + oa, plane, c->WBB, nB);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL);
+        {
+            TcGemm g = G0(nA, nB, nB);
+            setA(g, 0, lB, 0, 0, 1, 0, 1);
+            setB(g, 0, lB, 0, 1, 0, 1);
+            setC(g, 0, lB, 0, 1);
+            ops_cc(g, c->TAB, nB, c->WBB, nB, c->ZAB, nB);
+            g.alpha = -1.0;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(nA, nA, nB);
+            setA(g, 0, 1, 0, 0, nA, 0, 0);
+            setB(g, 0, 1, 0, lB, 0, 0);
+            setC(g, 0, lA, 0, 1);
+            ops_rc(g, c->KxBA, c->TAB, nB, c->WAA, nA);
+            g.alpha = 0.5;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(oa * oa, vb * vb, NQ);
+            setA(g, n, 1, oa, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, vb, 1);
+            setC(g, vb * lA, vb, 1, lA);
+            ops_cc(g, c->Lt[0], plane, c->Lt[1] + (long long)ob * n + ob, plane, c->WAA, nA);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        EW(c, k_add_Fd, (long long)oa * vb * vb + (long long)oa * oa * vb, oa, vb, n, c->Ft[0], oa, c->Ft[1], ob, c->WAA, lA, (long long)nA, 0LL, 0LL);
+        {
+            TcGemm g = G0(nB, nA, nA);
+            setA(g, 0, 1, 0, 0, lB, 0, 0);
+            setB(g, 0, lA, 0, 1, 0, 1);
+            setC(g, 0, lA, 0, 1);
+            ops_cc(g, c->TAB, nB, c->WAA, nA, c->ZBA, nA);
+            g.alpha = -1.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 11. ladders (pp with all-orbital rows; hh and the T1 corrections from the occupied rows)
+    if (c->timing && !c->capturing) { CK(cudaEventRecord(c->ev[0], st)); c->lad_flops = 0.0; }
+    double* lf = (c->timing && !c->capturing) ? &c->lad_flops : nullptr;
+    if (d.oo > 0) {
+        LadderArgs a;
+        a.LA = c->L[0]; a.LB = c->L[1]; a.sQA = a.sQB = nn; a.ldA = a.ldB = n; a.offA = d.o[0]; a.offB = d.o[1];
+        a.nA = a.nB = n; a.vA = d.v[0]; a.vB = d.v[1]; a.NQ = NQ;
+        a.X = c->Xab; a.ldX = 2LL * d.oo; a.N2 = 2 * d.oo; a.Y = c->Yab; a.ldY = 2LL * d.oo;
+        a.tiles = c->tiles_ab; a.ntiles = c->ntiles_ab;
+        c->launches += ladder_launch(a, st, &c->flops);
+        if (lf) ladder_launch_flops(a, lf);
+    }
+    for (int s = 0; s < 2; ++s) {
+        if (d.po[s] == 0) continue;
+        LadderArgs a;
+        a.LA = a.LB = c->L[s]; a.sQA = a.sQB = nn; a.ldA = a.ldB = n; a.offA = a.offB = d.o[s];
+        a.nA = a.nB = n; a.vA = a.vB = d.v[s]; a.NQ = NQ;
+        a.X = c->Xss[s]; a.ldX = 2LL * d.po[s]; a.N2 = 2 * d.po[s]; a.Y = c->Yss[s]; a.ldY = 2LL * d.po[s];
+        a.tiles = c->tiles_ss[s]; a.ntiles = c->ntiles_ss[s];
+        c->launches += ladder_launch(a, st, &c->flops);
+        if (lf) ladder_launch_flops(a, lf);
+    }
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], st));
+
+    if (d.oo > 0) {
+        const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], oo = d.oo;
+        const long long lY = 2LL * oo;
+        double* Yvv = c->Yab + ((long long)oa * n + ob) * lY;
+        {   // <mN||iJ>~ = sum_Q L~_mi L~_NJ
+            TcGemm g = G0(oa * oa, ob * ob, NQ);
+            setA(g, n, 1, oa, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, ob, 1);
+            setC(g, ob * lY, ob, lY, 1);
+            ops_cc(g, c->Lt[0], plane, c->Lt[1], plane, c->Wooab, oo);
+            run(c, g);
+        }
+        {   // + t_mN^aB <mN||iJ>~
+            TcGemm g = G0(va * vb, oo, oo);
+            setA(g, vb * lY, lY, vb, 0, 1, 0, 1);
+            setB(g, 0, lY, 0, 1, 0, 1);
+            setC(g, n * lY, lY, 0, 1);
+            ops_cc(g, c->Xab, oo, c->Wooab, oo, Yvv, oo);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // + tau_mN^aB Y_iJ^mN
+            TcGemm g = G0(va * vb, oo, oo);
+            setA(g, vb * lY, lY, vb, ob, 1, ob, 1);
+            setB(g, n * lY, lY, 0, 1, 0, 1);
+            setC(g, n * lY, lY, 0, 1);
+            ops_cc(g, c->tauab, oo, c->Yab, oo, Yvv, oo);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // - sum_m t_m^a Y_iJ^mB
+            TcGemm g = G0(va, vb * oo, oa);
+            setA(g, 0, 1, 0, 0, va, 0, 0);
+            setB(g, 0, n * lY, lY, 1, oo, 1);
+            setC(g, 0, n * lY, lY, 1);
+            ops_cc(g, c->t1r, n1, c->Yab + (long long)ob * lY, oo, Yvv, oo);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {   // - sum_N t_N^B Y_iJ^aN   (batched over a)
+            TcGemm g = G0(vb, oo, ob);
+            setA(g, 0, 1, 0, 0, vb, 0, 0);
+            setB(g, 0, lY, 0, 1, 0, 1);
+            setC(g, 0, lY, 0, 1);
+            ops_cc(g, c->t1r + d.n1a, n1, c->Yab + (long long)oa * n * lY, oo, Yvv, oo);
+            g.nsb = va; g.sbA = 0; g.sbB = n * lY; g.sbC = n * lY;
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+    }
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s], po = d.po[s];
+        const long long off1 = s ? d.n1a : 0;
+        if (po == 0) continue;
+        const long long lP = 2LL * po, o2 = (long long)o * o;
+        double* Yvv = c->Yss[s] + ((long long)o * n + o) * lP;
+        {
+            TcGemm g = G0(o * o, o * o, NQ);
+            setA(g, n, 1, o, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, o, 1);
+            setC(g, o * 2 * o2, o, 2 * o2, 1);
+            ops_cc(g, c->Lt[s], plane, c->Lt[s], plane, c->W4[s], o2);
+            run(c, g);
+        }
+        EW(c, k_ss_prep, (long long)po * po, o, po, n, c->opairs[s], c->W4[s], c->Yss[s], c->Wp[s], c->Yoop[s]);
+        {
+            TcGemm g = G0(v * v, po, po);
+            setA(g, v * lP, lP, v, 0, 1, 0, 1);
+            setB(g, 0, lP, 0, 1, 0, 1);
+            setC(g, n * lP, lP, 0, 1);
+            ops_cc(g, c->Xss[s], po, c->Wp[s], po, Yvv, po);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(v * v, po, po);
+            setA(g, v * lP, lP, v, 0, 1, 0, 1);
+            setB(g, 0, lP, 0, 1, 0, 1);
+            setC(g, n * lP, lP, 0, 1);
+            ops_cc(g, c->tauss[s], po, c->Yoop[s], po, Yvv, po);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // Zv[a][b] = sum_m t_m^a Y^{mb}
+            TcGemm g = G0(v, v * po, o);
+            setA(g, 0, 1, 0, 0, v, 0, 0);
+            setB(g, 0, n * lP, lP, 1, po, 1);
+            setC(g, 0, v * lP, lP, 1);
+            ops_cc(g, c->t1r + off1, n1, c->Yss[s] + (long long)o * lP, po, c->Zv[s], po);
+            run(c, g);
+        }
+    }
+
+    // ---- 12. antisymmetrise and write the packed residual
+    {
+        AsmArgs A;
+        A.Zsc = c->Zsc; A.ZAB = c->ZAB; A.ZBA = c->ZBA; A.Yab = c->Yab; A.r1buf = c->r1buf;
+        for (int s = 0; s < 2; ++s) {
+            A.Yss[s] = c->Yss[s]; A.Zv[s] = c->Zv[s]; A.Ft[s] = c->Ft[s];
+            A.opairs[s] = c->opairs[s]; A.vpairs[s] = c->vpairs[s];
+        }
+        A.r1p = r; A.r2p = r + 2 * d.n_t1;
+        EW(c, k_assemble, d.n_t1 + d.n_t2, d, A);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { c->cuda_err = (int)e; return RTCC_ECUDA; }
+    return RTCC_OK;
+}
+
+}  // namespace
+
+namespace {
+
+int copy_in(rtcc_ctx* c, double* dst, const double* src, long long ndoubles)
+{
+    if (ndoubles <= 0) return 0;
+    CK(cudaMemcpyAsync(dst, src, ndoubles * 8, (c->flags & RTCC_HOST_PTRS) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->st));
+    return 0;
+}
+int copy_out(const rtcc_ctx* cc, double* dst, const double* src, long long ndoubles)
+{
+    rtcc_ctx* c = const_cast<rtcc_ctx*>(cc);
+    if (ndoubles <= 0) return 0;
+    CK(cudaMemcpyAsync(dst, src, ndoubles * 8, (c->flags & RTCC_HOST_PTRS) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->st));
+    return 0;
+}
+
+// gr = R(gx), scal[0..1] = E; graph replay unless timing is on
+int eval_gx(rtcc_ctx* c)
+{
+    if (c->graph && !c->timing) {
+        CK(cudaGraphLaunch(c->graph, c->st));
+        c->launches += c->res_launches;
+        c->flops += c->res_flops;
+        return 0;
+    }
+    int rc = residual_pipeline(c, c->gx, c->gr);
+    return rc;
+}
+
+int read_scal(rtcc_ctx* c)
+{
+    CK(cudaMemcpyAsync(c->h_scal, c->scal, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return 0;
+}
+
+void model_ladder_flops(rtcc_ctx* c)
+{
+    // pp apply = 4[P(va)^2 P(oa) + P(vb)^2 P(ob) + (va vb)^2 oa ob],
+    //                 pp W-build = 2K[2P(va)^2 + 2P(vb)^2 + (va vb)^2]
+    const Dims& d = c->d;
+    double pva = d.pv[0], pvb = d.pv[1], vab = (double)d.v[0] * d.v[1];
+    c->lad_model = 4.0 * (pva * pva * d.po[0] + pvb * pvb * d.po[1] + vab * vab * d.oo)
+                 + 2.0 * d.NQ * (2.0 * pva * pva + 2.0 * pvb * pvb + vab * vab);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* rtcc_strerror(int code)
+{
+    switch (code) {
+        case RTCC_OK: return "ok";
+        case RTCC_EINVAL: return "invalid argument";
+        case RTCC_ENOMEM: return "out of memory";
+        case RTCC_ECUDA: return "CUDA error";
+        case RTCC_ENOCONV: return "micro-iterations did not converge";
+        case RTCC_ENONFINITE: return "non-finite amplitudes";
+        default: return "unknown error";
+    }
+}
+
+int rtcc_last_cuda_error(const rtcc_ctx* c) { return c ? c->cuda_err : 0; }
+
+void rtcc_destroy(rtcc_ctx* c)
+{
+    if (!c) return;
+    if (c->graph) cudaGraphExecDestroy(c->graph);
+    if (c->ev[0]) cudaEventDestroy(c->ev[0]);
+    if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+    for (void* p : c->allocs) cudaFree(p);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    delete c;
+}
+
+int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const double* L, const double* fock,
+                unsigned flags, void* cuda_stream)
+{
+    if (!out) return RTCC_EINVAL;
+    *out = nullptr;
+    if (!L || !fock || oa < 0 || ob < 0 || va < 1 || vb < 1 || NQ < 1 || oa + va != ob + vb || oa + ob < 1) return RTCC_EINVAL;
+    if ((long long)(oa + va) * (oa + va) * (long long)NQ >= (1LL << 40)) return RTCC_EINVAL;
+    rtcc_ctx* c = new (std::nothrow) rtcc_ctx();
+    if (!c) return RTCC_ENOMEM;
+    c->flags = flags;
+    c->st = (cudaStream_t)cuda_stream;
+    int rc = RTCC_OK;
+#define FAIL(code) do { rc = (code); goto fail; } while (0)
+#define CKC(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { c->cuda_err = (int)e_; rc = RTCC_ECUDA; goto fail; } } while (0)
+#define DA(p, cnt, name) do { int r_ = dalloc(c, &(p), (long long)(cnt), name); if (r_) { rc = r_; goto fail; } } while (0)
+    {
+        Dims& d = c->d;
+        d.o[0] = oa; d.o[1] = ob; d.v[0] = va; d.v[1] = vb; d.n = oa + va; d.NQ = NQ;
+        d.n1a = oa * va; d.n1b = ob * vb; d.n1 = d.n1a + d.n1b;
+        d.nA = oa * vb; d.nB = ob * va;
+        for (int s = 0; s < 2; ++s) { d.po[s] = d.o[s] * (d.o[s] - 1) / 2; d.pv[s] = d.v[s] * (d.v[s] - 1) / 2; }
+        d.oo = oa * ob;
+        d.off_t1[0] = 0; d.off_t1[1] = d.n1a;
+        d.off_t2[0] = 0; d.off_t2[1] = (long long)d.po[0] * d.pv[0];
+        d.off_t2[2] = d.off_t2[1] + (long long)d.po[1] * d.pv[1];
+        d.n_t1 = d.n1;
+        d.n_t2 = d.off_t2[2] + (long long)d.oo * va * vb;
+        c->namp = d.n_t1 + d.n_t2;
+        const int n = d.n, n1 = d.n1;
+        const long long nn = (long long)n * n, plane = (long long)NQ * nn;
+
+        int dev = 0;
+        CKC(cudaGetDevice(&dev));
+        CKC(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+        CKC(tcgemm_init());
+        CKC(ladder_init());
+        CKC(cudaEventCreate(&c->ev[0]));
+        CKC(cudaEventCreate(&c->ev[1]));
+        CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
+
+        for (int s = 0; s < 2; ++s) {
+            DA(c->L[s], plane, s ? "L1" : "L0");
+            DA(c->Lt[s], 2 * plane, s ? "Lt1" : "Lt0");
+            DA(c->fockd[s], nn, nullptr);
+            DA(c->Fb[s], nn, s ? "Fb1" : "Fb0");
+            DA(c->Ft[s], 2 * nn, s ? "Ft1" : "Ft0");
+            DA(c->Kx[s], (long long)d.o[s] * d.v[s] * d.o[s] * d.v[s], s ? "Kx1" : "Kx0");
+            const int po = d.po[s], v = d.v[s], o = d.o[s];
+            DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
+            DA(c->tauss[s], (long long)v * v * 2 * po, nullptr);
+            DA(c->Yss[s], nn * 2 * po, s ? "Yss1" : "Yss0");
+            DA(c->W4[s], (long long)o * o * 2 * o * o, nullptr);
+            DA(c->Wp[s], (long long)po * 2 * po, nullptr);
+            DA(c->Yoop[s], (long long)po * 2 * po, nullptr);
+            DA(c->Zv[s], (long long)v * v * 2 * po, s ? "Zv1" : "Zv0");
+            CKC(cudaMemsetAsync(c->Yss[s], 0, (size_t)(nn * 2 * po > 0 ? nn * 2 * po : 1) * 8, c->st));
+        }
+        DA(c->KxBA, (long long)d.nB * d.nA, "KxBA");
+        DA(c->t1r, 2LL * n1, "t1r");
+        DA(c->Tsc, 2LL * n1 * n1, "Tsc");
+        DA(c->Wsc, 2LL * n1 * n1, "Wsc");
+        DA(c->Zsc, 2LL * n1 * n1, "Zsc");
+        DA(c->TAB, 2LL * d.nA * d.nB, "TAB");
+        DA(c->WBB, 2LL * d.nB * d.nB, "WBB");
+        DA(c->WAA, 2LL * d.nA * d.nA, "WAA");
+        DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
+        DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
+        DA(c->Mq, 2LL * NQ * n1, "Mq");
+        DA(c->gam, 2LL * NQ, "gam");
+        DA(c->r1buf, 2LL * n1, "r1buf");
+        DA(c->Xab, (long long)va * vb * 2 * d.oo, "Xab");
+        DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
+        DA(c->Yab, nn * 2 * d.oo, "Yab");
+        DA(c->Wooab, (long long)d.oo * 2 * d.oo, nullptr);
+        c->ws_cap = 8LL << 20;
+        DA(c->ws, c->ws_cap, nullptr);
+        DA(c->partial, 2 * RED_BLOCKS, nullptr);
+        DA(c->bmax, RED_BLOCKS, nullptr);
+        DA(c->scal, 8, nullptr);
+        DA(c->gx, 2 * c->namp, "gx");
+        DA(c->gr, 2 * c->namp, "gr");
+        DA(c->t_cur, 2 * c->namp, nullptr);
+        DA(c->r_cur, 2 * c->namp, nullptr);
+        DA(c->Bv, 2 * c->namp, nullptr);
+        DA(c->Dn, c->namp, "Dn");
+
+        // inputs
+        const cudaMemcpyKind kin = (flags & RTCC_HOST_PTRS) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+        for (int s = 0; s < 2; ++s) {
+            CKC(cudaMemcpyAsync(c->L[s], L + s * plane, plane * 8, kin, c->st));
+            CKC(cudaMemcpyAsync(c->fockd[s], fock + s * nn, nn * 8, kin, c->st));
+        }
+        // pair tables and ladder row tiles
+        for (int s = 0; s < 2; ++s) {
+            std::vector<int2> op((size_t)(d.po[s] > 0 ? d.po[s] : 1)), vp((size_t)(d.pv[s] > 0 ? d.pv[s] : 1));
+            for (int j = 0; j < d.o[s]; ++j) for (int i = 0; i < j; ++i) op[(size_t)pair_index(i, j)] = make_int2(i, j);
+            for (int b = 0; b < d.v[s]; ++b) for (int a = 0; a < b; ++a) vp[(size_t)pair_index(a, b)] = make_int2(a, b);
+            DA(c->opairs[s], op.size(), nullptr);
+            DA(c->vpairs[s], vp.size(), nullptr);
+            CKC(cudaMemcpy(c->opairs[s], op.data(), op.size() * sizeof(int2), cudaMemcpyHostToDevice));
+            CKC(cudaMemcpy(c->vpairs[s], vp.data(), vp.size() * sizeof(int2), cudaMemcpyHostToDevice));
+        }
+        {
+            std::vector<int2> tab, tss;
+            for (int p0 = 0; p0 < n; p0 += LD_PP)
+                for (int q0 = 0; q0 < n; q0 += LD_PQ) {
+                    tab.push_back(make_int2(p0, q0));
+                    if (p0 <= q0) tss.push_back(make_int2(p0, q0));
+                }
+            DA(c->tiles_ab, tab.size(), nullptr);
+            CKC(cudaMemcpy(c->tiles_ab, tab.data(), tab.size() * sizeof(int2), cudaMemcpyHostToDevice));
+            c->ntiles_ab = (int)tab.size();
+            for (int s = 0; s < 2; ++s) {
+                DA(c->tiles_ss[s], tss.size(), nullptr);
+                CKC(cudaMemcpy(c->tiles_ss[s], tss.data(), tss.size() * sizeof(int2), cudaMemcpyHostToDevice));
+                c->ntiles_ss[s] = (int)tss.size();
+            }
+        }
+        // constant integral blocks: Kx (exchange-type oovv), K_bare added to the Fock matrix
+        for (int s = 0; s < 2; ++s) {
+            const int o = d.o[s], v = d.v[s], n1s = o * v;
+            CKC(cudaMemcpyAsync(c->Fb[s], c->fockd[s], nn * 8, cudaMemcpyDeviceToDevice, c->st));
+            if (o == 0) continue;
+            {
+                TcGemm g = G0(n1s, n1s, NQ);
+                setA(g, n, 1, v, 0, nn, 0, 0);
+                setB(g, 0, nn, n, 1, v, 1);
+                setC(g, (long long)v * n1s, 1, v, n1s);
+                ops_rr(g, c->L[s] + o, c->L[s] + o, c->Kx[s]);
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(n, n, NQ * o);
+                setA(g, 0, n, 0, nn, 1, o, 1);
+                setB(g, nn, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_rr(g, c->L[s], c->L[s], c->Fb[s]);
+                g.beta = 1.0;
+                run(c, g);
+            }
+        }
+        if (d.nA > 0 && d.nB > 0) {
+            TcGemm g = G0(ob * vb, oa * va, NQ);
+            setA(g, n, 1, vb, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, va, 1);
+            setC(g, (long long)va * d.nA, 1, vb, d.nA);
+            ops_rr(g, c->L[1] + ob, c->L[0] + oa, c->KxBA);
+            run(c, g);
+        }
+        EW(c, k_build_Dn, c->namp, d, c->fockd[0], c->fockd[1], c->opairs[0], c->opairs[1], c->vpairs[0], c->vpairs[1], c->Dn);
+        CKC(cudaMemsetAsync(c->t_cur, 0, (size_t)c->namp * 16, c->st));
+        CKC(cudaMemsetAsync(c->gx, 0, (size_t)c->namp * 16, c->st));
+        model_ladder_flops(c);
+
+        // R(T=0), E(T=0); count the launches / flops of one evaluation; then capture it as a graph
+        {
+            long long l0 = c->launches; double f0 = c->flops;
+            rc = residual_pipeline(c, c->gx, c->gr);
+            if (rc) goto fail;
+            c->res_launches = c->launches - l0; c->res_flops = c->flops - f0;
+            CKC(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+            if (read_scal(c)) { rc = RTCC_ECUDA; goto fail; }
+            c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
+        }
+        if (!getenv("RTCC_NO_GRAPH")) {
+            cudaStream_t cs = nullptr;
+            cudaStream_t user = c->st;
+            CKC(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+            long long l0 = c->launches; double f0 = c->flops;
+            c->st = cs; c->capturing = true;
+            cudaGraph_t gph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+            int prc = RTCC_OK;
+            if (e == cudaSuccess) {
+                prc = residual_pipeline(c, c->gx, c->gr);
+                e = cudaStreamEndCapture(cs, &gph);
+            }
+            c->st = user; c->capturing = false;
+            c->launches = l0; c->flops = f0;
+            if (e == cudaSuccess && prc == RTCC_OK && gph) e = cudaGraphInstantiate(&c->graph, gph, 0);
+            if (gph) cudaGraphDestroy(gph);
+            cudaStreamDestroy(cs);
+            if (e != cudaSuccess || prc != RTCC_OK) { c->cuda_err = (int)e; rc = RTCC_ECUDA; goto fail; }
+        }
+        CKC(cudaStreamSynchronize(c->st));
+    }
+    *out = c;
+    return RTCC_OK;
+fail:
+    cudaGetLastError();
+    rtcc_destroy(c);
+    return rc;
+#undef FAIL
+#undef CKC
+#undef DA
+}
+
+int rtcc_sizes(const rtcc_ctx* c, long long* n_t1, long long* n_t2, long long* workspace_bytes)
+{
+    if (!c) return RTCC_EINVAL;
+    if (n_t1) *n_t1 = c->d.n_t1;
+    if (n_t2) *n_t2 = c->d.n_t2;
+    if (workspace_bytes) *workspace_bytes = c->bytes;
+    return RTCC_OK;
+}
+
+int rtcc_residual(rtcc_ctx* c, const double* t1, const double* t2, double* r1, double* r2)
+{
+    if (!c || !t1 || !t2 || !r1 || !r2) return RTCC_EINVAL;
+    const Dims& d = c->d;
+    if (copy_in(c, c->gx, t1, 2 * d.n_t1)) return RTCC_ECUDA;
+    if (copy_in(c, c->gx + 2 * d.n_t1, t2, 2 * d.n_t2)) return RTCC_ECUDA;
+    int rc = eval_gx(c);
+    if (rc) return rc;
+    if (copy_out(c, r1, c->gr, 2 * d.n_t1)) return RTCC_ECUDA;
+    if (copy_out(c, r2, c->gr + 2 * d.n_t1, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (read_scal(c)) return RTCC_ECUDA;
+    c->E_res[0] = c->h_scal[0]; c->E_res[1] = c->h_scal[1];
+    if (c->timing) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+        c->lad_ms = ms;
+    }
+    return RTCC_OK;
+}
+
+int rtcc_residual_energy(const rtcc_ctx* c, double out[2])
+{
+    if (!c || !out) return RTCC_EINVAL;
+    out[0] = c->E_res[0]; out[1] = c->E_res[1];
+    return RTCC_OK;
+}
+
+int rtcc_set_amplitudes(rtcc_ctx* c, const double* t1, const double* t2, double time, const double cc[2])
+{
+    if (!c || !t1 || !t2 || !cc || !std::isfinite(time)) return RTCC_EINVAL;
+    const Dims& d = c->d;
+    if (copy_in(c, c->gx, t1, 2 * d.n_t1)) return RTCC_ECUDA;
+    if (copy_in(c, c->gx + 2 * d.n_t1, t2, 2 * d.n_t2)) return RTCC_ECUDA;
+    int rc = eval_gx(c);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->t_cur, c->gx, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    if (read_scal(c)) return RTCC_ECUDA;
+    c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
+    c->time = time; c->C[0] = cc[0]; c->C[1] = cc[1];
+    return RTCC_OK;
+}
+
+int rtcc_get_amplitudes(const rtcc_ctx* c, double* t1, double* t2)
+{
+    if (!c || !t1 || !t2) return RTCC_EINVAL;
+    const Dims& d = c->d;
+    if (copy_out(c, t1, c->t_cur, 2 * d.n_t1)) return RTCC_ECUDA;
+    if (copy_out(c, t2, c->t_cur + 2 * d.n_t1, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (cudaStreamSynchronize(c->st) != cudaSuccess) return RTCC_ECUDA;
+    return RTCC_OK;
+}
+
+int rtcc_set_solver(rtcc_ctx* c, int mode, double tol, int max_micro, int fixed_micro)
+{
+    if (!c || (mode != 0 && mode != 1) || !(tol > 0.0) || max_micro < 1 || fixed_micro < 0) return RTCC_EINVAL;
+    c->mode = mode; c->tol = tol; c->max_micro = max_micro; c->fixed_micro = fixed_micro;
+    return RTCC_OK;
+}
+
+int rtcc_step(rtcc_ctx* c, double dt)
+{
+    if (!c || !std::isfinite(dt)) return RTCC_EINVAL;
+    const long long N = c->namp;
+    const double hh = 0.5 * dt;
+    // B = t + (i dt/2) R(t)
+    k_caxpy<<<nblk(N, c->num_sms * 16), 256, 0, c->st>>>(N, c->t_cur, c->r_cur, 0.0, hh, c->Bv);
+    c->launches++;
+    int k = 0;
+    double E_new[2] = {0, 0};
+    for (;;) {
+        const double* xin = k == 0 ? c->t_cur : c->gx;
+        const double* rin = k == 0 ? c->r_cur : c->gr;
+        k_am_update<<<RED_BLOCKS, RED_THREADS, 0, c->st>>>(N, c->Bv, rin, xin, c->Dn, c->mode, hh, c->gx, c->bmax);
+        k_max_partials<<<1, 32, 0, c->st>>>(c->bmax, RED_BLOCKS, c->scal + 2);
+        c->launches += 2;
+        ++k;
+        const bool last_fixed = c->fixed_micro > 0 && k >= c->fixed_micro;
+        if (c->fixed_micro == 0 || last_fixed) {
+            // delta decides (or, in fixed mode, is checked once at the end)
+            if (c->fixed_micro == 0) {
+                if (read_scal(c)) return RTCC_ECUDA;
+                if (!std::isfinite(c->h_scal[2])) return RTCC_ENONFINITE;
+            }
+        }
+        int rc = eval_gx(c);
+        if (rc) return rc;
+        if (c->fixed_micro > 0) {
+            if (last_fixed) break;
+        } else if (c->h_scal[2] < c->tol) {
+            break;
+        } else if (k >= c->max_micro) {
+            return RTCC_ENOCONV;
+        }
+    }
+    if (read_scal(c)) return RTCC_ECUDA;
+    if (!std::isfinite(c->h_scal[2]) || !std::isfinite(c->h_scal[0]) || !std::isfinite(c->h_scal[1])) return RTCC_ENONFINITE;
+    E_new[0] = c->h_scal[0]; E_new[1] = c->h_scal[1];
+    // C += (i dt/2) (E_old + E_new)
+    const double sr = c->E[0] + E_new[0], si = c->E[1] + E_new[1];
+    c->C[0] += -hh * si;
+    c->C[1] += hh * sr;
+    CK(cudaMemcpyAsync(c->t_cur, c->gx, (size_t)N * 16, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)N * 16, cudaMemcpyDeviceToDevice, c->st));
+    c->E[0] = E_new[0]; c->E[1] = E_new[1];
+    c->time += dt;
+    c->last_micro = k;
+    return RTCC_OK;
+}
+
+int rtcc_cumulant(const rtcc_ctx* c, double out[4])
+{
+    if (!c || !out) return RTCC_EINVAL;
+    out[0] = c->C[0]; out[1] = c->C[1]; out[2] = c->E[0]; out[3] = c->E[1];
+    return RTCC_OK;
+}
+
+int rtcc_last_micro_iterations(const rtcc_ctx* c) { return c ? c->last_micro : RTCC_EINVAL; }
+double rtcc_time(const rtcc_ctx* c) { return c ? c->time : 0.0; }
+
+int rtcc_counters(const rtcc_ctx* c, long long* launches, double* flops)
+{
+    if (!c) return RTCC_EINVAL;
+    if (launches) *launches = c->launches;
+    if (flops) *flops = c->flops;
+    return RTCC_OK;
+}
+int rtcc_reset_counters(rtcc_ctx* c)
+{
+    if (!c) return RTCC_EINVAL;
+    c->launches = 0; c->flops = 0.0;
+    return RTCC_OK;
+}
+int rtcc_set_timing(rtcc_ctx* c, int on)
+{
+    if (!c) return RTCC_EINVAL;
+    c->timing = on ? 1 : 0;
+    return RTCC_OK;
+}
+int rtcc_ladder_timing(const rtcc_ctx* c, double* ms, double* flops, double* model_flops)
+{
+    if (!c) return RTCC_EINVAL;
+    if (ms) *ms = c->lad_ms;
+    if (flops) *flops = c->lad_flops;
+    if (model_flops) *model_flops = c->lad_model;
+    return RTCC_OK;
+}
+
+int rtcc_fp64_peak(double* tflops)
+{
+    if (!tflops) return RTCC_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return RTCC_ECUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return RTCC_ECUDA;
+    double* buf = nullptr;
+    const int grid = sms * 2, iters = 4000;
+    if (cudaMalloc(&buf, (size_t)grid * 256 * 8) != cudaSuccess) return RTCC_ENOMEM;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        k_dmma_peak<<<grid, 256>>>(buf, iters, 1e-9);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (cudaGetLastError() != cudaSuccess) return RTCC_ECUDA;
+    const double fl = 16.0 * 2.0 * 8 * 8 * 4 * (double)iters * 8.0 * grid;
+    *tflops = fl / (best * 1e-3) * 1e-12;
+    return RTCC_OK;
+}
+
+long long rtcc_debug_buffer(const rtcc_ctx* c, const char* name, double* out, long long max_doubles)
+{
+    if (!c || !name) return RTCC_EINVAL;
+    for (auto& kv : c->named)
+        if (kv.first == name) {
+            long long cnt = kv.second.second;
+            if (out && max_doubles > 0) {
+                long long m = cnt < max_doubles ? cnt : max_doubles;
+                if (cudaMemcpy(out, kv.second.first, (size_t)m * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return RTCC_ECUDA;
+            }
+            return cnt;
+        }
+    return RTCC_EINVAL;
+}
+
+int rtcc_debug_gemm(int M, int N, int K, const double* A, const double* B, double* C, double alpha, double beta, int cplx)
+{
+    if (M < 1 || N < 1 || K < 0 || !A || !B || !C) return RTCC_EINVAL;
+    const int np = cplx ? 2 : 1;
+    double *dA = nullptr, *dB = nullptr, *dC = nullptr, *ws = nullptr;
+    int sms = 148, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long wscap = 4LL << 20;
+    if (cudaMalloc(&dA, (size_t)np * M * (K > 0 ? K : 1) * 8) != cudaSuccess || cudaMalloc(&dB, (size_t)np * (K > 0 ? K : 1) * N * 8) != cudaSuccess ||
+        cudaMalloc(&dC, (size_t)np * M * N * 8) != cudaSuccess || cudaMalloc(&ws, wscap * 8) != cudaSuccess) {
+        cudaFree(dA); cudaFree(dB); cudaFree(dC); cudaFree(ws);
+        return RTCC_ENOMEM;
+    }
+    cudaMemcpy(dA, A, (size_t)np * M * K * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(dB, B, (size_t)np * K * N * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(dC, C, (size_t)np * M * N * 8, cudaMemcpyHostToDevice);
+    tcgemm_init();
+    TcGemm g = G0(M, N, K);
+    setA(g, 0, K, 0, 0, 1, 0, 1);
+    setB(g, 0, N, 0, 1, 0, 1);
+    setC(g, 0, N, 0, 1);
+    if (cplx) ops_cc(g, dA, (long long)M * K, dB, (long long)K * N, dC, (long long)M * N);
+    else ops_rr(g, dA, dB, dC);
+    g.alpha = alpha; g.beta = beta; g.ws = ws;
+    tcgemm_launch(g, nullptr, wscap, sms, nullptr);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(C, dC, (size_t)np * M * N * 8, cudaMemcpyDeviceToHost);
+    cudaFree(dA); cudaFree(dB); cudaFree(dC); cudaFree(ws);
+    return e == cudaSuccess ? RTCC_OK : RTCC_ECUDA;
+}
+
+}  // extern "C"

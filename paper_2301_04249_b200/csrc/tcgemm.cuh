@@ -1,0 +1,322 @@
+// tcgemm.cuh -- FP64 tensor-core (DMMA m8n8k4) tensor-contraction GEMM for sm_100a.
+//
+// C(m,n) = alpha * sum_phases s_p * sum_k A_p(m,k) B_p(k,n) + beta * C(m,n)
+//
+// Every index of the three operands is a two-level index (hi,lo) with independent strides, so a
+// contraction over e.g. k=(Q,i) or an output scattered as [(m,e)][(j,b)] needs no transposition
+// pass.  Up to two phases with signs implement complex products on planar (Re/Im) storage:
+//   Re C = A_re B_re - A_im B_im,   Im C = A_re B_im + A_im B_re        (real integrals x complex
+//   amplitudes need one phase only; "mixed real-complex contractions").
+// Operands are staged global -> shared with 8-byte cp.async (zero-filled out of range: no
+// alignment or size restrictions), three stages deep; fragments are read with conflict-free
+// 64-bit LDS (row pitch == 4 mod 16 doubles) and fed to mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4, the
+// only FP64 tensor shape sm_100a has -- tcgen05 has no f64 kind).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rtcc {
+
+constexpr int TG_MAXB = 4;
+
+struct TcGemm {
+    int M, N, K;
+    int Mlo, Nlo, Klo;                       // extents of the "lo" part of each index (>=1)
+    long long am_hi, am_lo, ak_hi, ak_lo;    // A(m,k) strides
+    long long bk_hi, bk_lo, bn_hi, bn_lo;    // B(k,n) strides
+    long long cm_hi, cm_lo, cn_hi, cn_lo;    // C(m,n) strides
+    int nb;                                  // descriptor batches (<= TG_MAXB)
+    const double* A[TG_MAXB][2];
+    const double* B[TG_MAXB][2];
+    double* C[TG_MAXB];
+    signed char nphase[TG_MAXB], s0[TG_MAXB], s1[TG_MAXB];
+    int nsb;                                 // strided batches
+    long long sbA, sbB, sbC;
+    double alpha, beta;
+    int a_kfast, b_nfast;                    // which index of A / B is contiguous in memory
+    int ksplit;                              // deterministic split-K (partials in ws, reduced by a 2nd kernel)
+    double* ws;
+};
+
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, bool valid)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(d), "l"(gsrc), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ long long idx2(int x, int lo, long long s_hi, long long s_lo)
+{
+    if (lo >= 0x40000000) return (long long)x * s_lo;   // single-level fast path
+    int h = x / lo;
+    return (long long)h * s_hi + (long long)(x - h * lo) * s_lo;
+}
+
+template <int BM, int BN, int WM, int WN>
+__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32) tcgemm_kernel(const TcGemm g)
+{
+    constexpr int BK = 16, ST = 3;
+    constexpr int NTH = (BM / WM) * (BN / WN) * 32;
+    constexpr int LDA = BK + 4, LDB = BN + 4;
+    constexpr int EA = BM * BK / NTH, EB = BK * BN / NTH;
+    constexpr int TM = WM / 8, TN = WN / 8;
+    extern __shared__ double smem[];
+    double* As = smem;                        // [ST][BM][LDA]
+    double* Bs = smem + ST * BM * LDA;        // [ST][BK][LDB]
+    long long* rowA = (long long*)(Bs + ST * BK * LDB);   // [BM] offsets (or -1)
+    long long* colB = rowA + BM;                          // [BN]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int z = blockIdx.z;
+    const int split = z % g.ksplit; z /= g.ksplit;
+    const int sb = z % g.nsb;
+    const int db = z / g.nsb;
+    const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+
+    for (int i = tid; i < BM; i += NTH) {
+        int m = m0 + i;
+        rowA[i] = (m < g.M) ? idx2(m, g.Mlo, g.am_hi, g.am_lo) : -1;
+    }
+    for (int i = tid; i < BN; i += NTH) {
+        int n = n0 + i;
+        colB[i] = (n < g.N) ? idx2(n, g.Nlo, g.bn_hi, g.bn_lo) : -1;
+    }
+    __syncthreads();
+
+    const int nkt = (g.K + BK - 1) / BK;
+    const int per = (nkt + g.ksplit - 1) / g.ksplit;
+    const int kt0 = split * per;
+    const int kt1 = min(nkt, kt0 + per);
+    const int nk = max(kt1 - kt0, 0);
+    const int nph = g.nphase[db];
+    const int total = nk * nph;
+
+    const double* Ap[2] = {g.A[db][0] + sb * g.sbA, g.A[db][1] + sb * g.sbA};
+    const double* Bp[2] = {g.B[db][0] + sb * g.sbB, g.B[db][1] + sb * g.sbB};
+
+    auto load_tile = [&](int t, int stage) {
+        const int ph = t / nk;
+        const int kbase = (kt0 + (t - ph * nk)) * BK;
+        const double* A = Ap[ph];
+        const double* B = Bp[ph];
+        double* as = As + stage * BM * LDA;
+        double* bs = Bs + stage * BK * LDB;
+        if (g.a_kfast) {
+            const int kk = tid % BK, r0 = tid / BK;
+            const int k = kbase + kk;
+            const bool kv = k < g.K;
+            const long long ko = kv ? idx2(k, g.Klo, g.ak_hi, g.ak_lo) : 0;
+#pragma unroll
+            for (int j = 0; j < EA; ++j) {
+                int r = r0 + j * (NTH / BK);
+                long long ro = rowA[r];
+                bool v = kv && ro >= 0;
+                cp_async8(as + r * LDA + kk, v ? (A + ro + ko) : A, v);
+            }
+        } else {
+            const int r = tid % BM, k0 = tid / BM;
+            const long long ro = rowA[r];
+#pragma unroll
+            for (int j = 0; j < EA; ++j) {
+                int kk = k0 + j * (NTH / BM);
+                int k = kbase + kk;
+                bool v = (k < g.K) && ro >= 0;
+                long long ko = v ? idx2(k, g.Klo, g.ak_hi, g.ak_lo) : 0;
+                cp_async8(as + r * LDA + kk, v ? (A + ro + ko) : A, v);
+            }
+        }
+        if (g.b_nfast) {
+            const int c = tid % BN, k0 = tid / BN;
+            const long long co = colB[c];
+#pragma unroll
+            for (int j = 0; j < EB; ++j) {
+                int kk = k0 + j * (NTH / BN);
+                int k = kbase + kk;
+                bool v = (k < g.K) && co >= 0;
+                long long ko = v ? idx2(k, g.Klo, g.bk_hi, g.bk_lo) : 0;
+                cp_async8(bs + kk * LDB + c, v ? (B + co + ko) : B, v);
+            }
+        } else {
+            const int kk = tid % BK, c0 = tid / BK;
+            const int k = kbase + kk;
+            const bool kv = k < g.K;
+            const long long ko = kv ? idx2(k, g.Klo, g.bk_hi, g.bk_lo) : 0;
+#pragma unroll
+            for (int j = 0; j < EB; ++j) {
+                int c = c0 + j * (NTH / BK);
+                long long co = colB[c];
+                bool v = kv && co >= 0;
+                cp_async8(bs + kk * LDB + c, v ? (B + co + ko) : B, v);
+            }
+        }
+    };
+
+    double acc[TM][TN][2];
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    const int wm0 = (warp / (BN / WN)) * WM, wn0 = (warp % (BN / WN)) * WN;
+    const int lr = lane >> 2, lc = lane & 3;
+
+#pragma unroll
+    for (int s = 0; s < ST - 1; ++s) {
+        if (s < total) load_tile(s, s);
+        cp_async_commit();
+    }
+    for (int t = 0; t < total; ++t) {
+        cp_async_wait<ST - 2>();
+        __syncthreads();
+        {
+            int tn = t + ST - 1;
+            if (tn < total) load_tile(tn, tn % ST);
+            cp_async_commit();
+        }
+        if (nph == 2 && t == nk && g.s0[db] != g.s1[db]) {
+#pragma unroll
+            for (int i = 0; i < TM; ++i)
+#pragma unroll
+                for (int j = 0; j < TN; ++j) { acc[i][j][0] = -acc[i][j][0]; acc[i][j][1] = -acc[i][j][1]; }
+        }
+        const double* as = As + (t % ST) * BM * LDA;
+        const double* bs = Bs + (t % ST) * BK * LDB;
+#pragma unroll
+        for (int ks = 0; ks < BK / 4; ++ks) {
+            double a[TM], b[TN];
+#pragma unroll
+            for (int i = 0; i < TM; ++i) a[i] = as[(wm0 + 8 * i + lr) * LDA + ks * 4 + lc];
+#pragma unroll
+            for (int j = 0; j < TN; ++j) b[j] = bs[(ks * 4 + lc) * LDB + wn0 + 8 * j + lr];
+#pragma unroll
+            for (int i = 0; i < TM; ++i)
+#pragma unroll
+                for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_async_wait<0>();
+
+    const double sgn = (nph == 2) ? (double)g.s1[db] : (double)g.s0[db];
+    if (g.ksplit > 1) {
+        double* W = g.ws + ((long long)(db * g.nsb + sb) * g.ksplit + split) * (long long)g.M * g.N;
+#pragma unroll
+        for (int i = 0; i < TM; ++i) {
+            int m = m0 + wm0 + 8 * i + lr;
+            if (m >= g.M) continue;
+#pragma unroll
+            for (int j = 0; j < TN; ++j) {
+                int n = n0 + wn0 + 8 * j + 2 * lc;
+                if (n < g.N) W[(long long)m * g.N + n] = sgn * acc[i][j][0];
+                if (n + 1 < g.N) W[(long long)m * g.N + n + 1] = sgn * acc[i][j][1];
+            }
+        }
+        return;
+    }
+    double* C = g.C[db] + sb * g.sbC;
+    const double al = g.alpha * sgn, be = g.beta;
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+        int m = m0 + wm0 + 8 * i + lr;
+        if (m >= g.M) continue;
+        long long mo = idx2(m, g.Mlo, g.cm_hi, g.cm_lo);
+#pragma unroll
+        for (int j = 0; j < TN; ++j) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                int n = n0 + wn0 + 8 * j + 2 * lc + e;
+                if (n < g.N) {
+                    double* p = C + mo + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+                    double v = al * acc[i][j][e];
+                    if (be != 0.0) v += be * *p;
+                    *p = v;
+                }
+            }
+        }
+    }
+}
+
+// C = alpha * sum_splits ws + beta * C   (fixed summation order: deterministic)
+__global__ void tcgemm_splitk_reduce(const TcGemm g)
+{
+    const long long MN = (long long)g.M * g.N;
+    const int nbt = g.nb * g.nsb;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < MN * nbt; e += (long long)gridDim.x * blockDim.x) {
+        int bt = (int)(e / MN);
+        long long r = e - bt * MN;
+        int m = (int)(r / g.N), n = (int)(r - (long long)m * g.N);
+        int db = bt / g.nsb, sb = bt - db * g.nsb;
+        const double* W = g.ws + (long long)bt * g.ksplit * MN + r;
+        double s = 0.0;
+        for (int k = 0; k < g.ksplit; ++k) s += W[k * MN];
+        double* p = g.C[db] + sb * g.sbC + idx2(m, g.Mlo, g.cm_hi, g.cm_lo) + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+        double v = g.alpha * s;
+        if (g.beta != 0.0) v += g.beta * *p;
+        *p = v;
+    }
+}
+
+template <int BM, int BN> constexpr size_t tcgemm_smem()
+{
+    return sizeof(double) * (3 * BM * (16 + 4) + 3 * 16 * (BN + 4)) + sizeof(long long) * (BM + BN);
+}
+
+// Host launcher.  ws_cap = capacity (doubles) of g.ws; returns number of kernels launched (1 or 2).
+inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sms, double* flops_out = nullptr)
+{
+    if (g.M <= 0 || g.N <= 0 || g.nb <= 0 || g.nsb <= 0) return 0;
+    if (g.Mlo <= 0 || g.Mlo >= g.M) g.Mlo = 0x40000000;
+    if (g.Nlo <= 0 || g.Nlo >= g.N) g.Nlo = 0x40000000;
+    if (g.Klo <= 0 || g.Klo >= g.K) g.Klo = 0x40000000;
+    const int nbt = g.nb * g.nsb;
+    const long long t128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * nbt;
+    const bool big = t128 >= (long long)(num_sms * 3) / 4 && g.M > 64 && g.N > 64;
+    const int BM = big ? 128 : 64, BN = big ? 128 : 64;
+    const long long tiles = (long long)((g.M + BM - 1) / BM) * ((g.N + BN - 1) / BN) * nbt;
+    const int nkt = (g.K + 15) / 16;
+    int ks = 1;
+    if (g.ws && tiles * 2 <= num_sms && nkt >= 16) {
+        ks = (int)(num_sms / tiles);
+        if (ks > nkt / 8) ks = nkt / 8;
+        while (ks > 1 && (long long)ks * nbt * g.M * g.N > ws_cap) --ks;
+        if (ks < 1) ks = 1;
+    }
+    g.ksplit = ks;
+    if (flops_out) {
+        int tot_ph = 0;
+        for (int b = 0; b < g.nb; ++b) tot_ph += g.nphase[b];
+        *flops_out += 2.0 * g.M * g.N * (double)g.K * tot_ph * g.nsb;
+    }
+    dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, nbt * ks);
+    if (big) {
+        tcgemm_kernel<128, 128, 64, 32><<<grid, 256, tcgemm_smem<128, 128>(), st>>>(g);
+    } else {
+        tcgemm_kernel<64, 64, 32, 32><<<grid, 128, tcgemm_smem<64, 64>(), st>>>(g);
+    }
+    if (ks > 1) {
+        long long tot = (long long)g.M * g.N * nbt;
+        int blocks = (int)((tot + 255) / 256);
+        if (blocks > num_sms * 8) blocks = num_sms * 8;
+        tcgemm_splitk_reduce<<<blocks, 256, 0, st>>>(g);
+        return 2;
+    }
+    return 1;
+}
+
+inline cudaError_t tcgemm_init()
+{
+    cudaError_t e = cudaFuncSetAttribute(tcgemm_kernel<128, 128, 64, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)tcgemm_smem<128, 128>());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(tcgemm_kernel<64, 64, 32, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)tcgemm_smem<64, 64>());
+}
+
+}  // namespace rtcc

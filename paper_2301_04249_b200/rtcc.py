@@ -1,0 +1,227 @@
+"""Thin ctypes binding of librtcc (include/rtcc.h): argument marshalling only -- every step of the hot path
+runs in the CUDA kernels behind the C ABI.  There is no CPU fallback: if the library is missing or a call
+fails, an exception is raised.
+
+Arrays may be numpy arrays (the context is then created with RTCC_HOST_PTRS and the library copies) or
+torch CUDA tensors (device pointers, no copies).  Complex arrays are complex128.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "librtcc.so")
+_lib = None
+
+RTCC_HOST_PTRS = 1
+SYMBOLS = [
+    "rtcc_create", "rtcc_destroy", "rtcc_sizes", "rtcc_residual", "rtcc_residual_energy", "rtcc_set_amplitudes",
+    "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
+    "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
+    "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror",
+]
+
+
+class RtccError(RuntimeError):
+    def __init__(self, code, what, cuda=0):
+        super().__init__(f"{what}: error {code} ({strerror(code)})" + (f", cudaError {cuda}" if cuda else ""))
+        self.code = code
+
+
+def load():
+    """dlopen librtcc.so (built by paper_2301_04249_b200.build / __graft_entry__.build); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise RuntimeError(f"{_LIBPATH} not found: run `python -m paper_2301_04249_b200.build` (no CPU fallback exists)")
+        lib = ctypes.CDLL(_LIBPATH)
+        vp, i, d, ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
+        P = ctypes.POINTER
+        lib.rtcc_create.argtypes = [P(vp), i, i, i, i, i, vp, vp, ctypes.c_uint, vp]
+        lib.rtcc_destroy.argtypes = [vp]; lib.rtcc_destroy.restype = None
+        lib.rtcc_sizes.argtypes = [vp, P(ll), P(ll), P(ll)]
+        lib.rtcc_residual.argtypes = [vp, vp, vp, vp, vp]
+        lib.rtcc_residual_energy.argtypes = [vp, P(d)]
+        lib.rtcc_set_amplitudes.argtypes = [vp, vp, vp, d, P(d)]
+        lib.rtcc_get_amplitudes.argtypes = [vp, vp, vp]
+        lib.rtcc_set_solver.argtypes = [vp, i, d, i, i]
+        lib.rtcc_step.argtypes = [vp, d]
+        lib.rtcc_cumulant.argtypes = [vp, P(d)]
+        lib.rtcc_last_micro_iterations.argtypes = [vp]
+        lib.rtcc_time.argtypes = [vp]; lib.rtcc_time.restype = d
+        lib.rtcc_counters.argtypes = [vp, P(ll), P(d)]
+        lib.rtcc_reset_counters.argtypes = [vp]
+        lib.rtcc_set_timing.argtypes = [vp, i]
+        lib.rtcc_ladder_timing.argtypes = [vp, P(d), P(d), P(d)]
+        lib.rtcc_fp64_peak.argtypes = [P(d)]
+        lib.rtcc_debug_buffer.argtypes = [vp, ctypes.c_char_p, vp, ll]; lib.rtcc_debug_buffer.restype = ll
+        lib.rtcc_debug_gemm.argtypes = [i, i, i, vp, vp, vp, d, d, i]
+        lib.rtcc_last_cuda_error.argtypes = [vp]
+        lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return load().rtcc_strerror(int(code)).decode()
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _ptr(x):
+    if _is_torch(x):
+        return ctypes.c_void_p(x.data_ptr())
+    return ctypes.c_void_p(x.ctypes.data)
+
+
+def fp64_peak() -> float:
+    """Measured FP64 DMMA peak of the current device in TFLOP/s."""
+    v = ctypes.c_double(0.0)
+    rc = load().rtcc_fp64_peak(ctypes.byref(v))
+    if rc:
+        raise RtccError(rc, "rtcc_fp64_peak")
+    return v.value
+
+
+def debug_gemm(A: np.ndarray, B: np.ndarray, C: np.ndarray | None = None, alpha=1.0, beta=0.0):
+    """Test hook: alpha*A@B + beta*C through the tensor-core contraction kernel (real or complex128)."""
+    cplx = np.iscomplexobj(A) or np.iscomplexobj(B)
+    M, K = A.shape
+    N = B.shape[1]
+    if cplx:
+        pa = np.ascontiguousarray(np.stack([A.real, A.imag]).astype(np.float64))
+        pb = np.ascontiguousarray(np.stack([B.real, B.imag]).astype(np.float64))
+        pc = np.zeros((2, M, N)) if C is None else np.ascontiguousarray(np.stack([C.real, C.imag]).astype(np.float64))
+    else:
+        pa = np.ascontiguousarray(A, dtype=np.float64)
+        pb = np.ascontiguousarray(B, dtype=np.float64)
+        pc = np.zeros((M, N)) if C is None else np.array(C, dtype=np.float64)
+    rc = load().rtcc_debug_gemm(M, N, K, _ptr(pa), _ptr(pb), _ptr(pc), float(alpha), float(beta), int(cplx))
+    if rc:
+        raise RtccError(rc, "rtcc_debug_gemm")
+    return pc[0] + 1j * pc[1] if cplx else pc
+
+
+class Rtcc:
+    """One (N-1)-electron RT-EOM-CCSD problem on the current CUDA device (see include/rtcc.h)."""
+
+    def __init__(self, oa, ob, va, vb, n_chol, L, fock, stream=None):
+        lib = load()
+        self._lib = lib
+        self.device_mode = _is_torch(L)
+        if self.device_mode:
+            import torch
+            assert L.is_cuda and fock.is_cuda and L.dtype == torch.float64 and L.is_contiguous() and fock.is_contiguous()
+        else:
+            L = np.ascontiguousarray(L, dtype=np.float64)
+            fock = np.ascontiguousarray(fock, dtype=np.float64)
+        self.dims = (oa, ob, va, vb, n_chol)
+        h = ctypes.c_void_p()
+        flags = 0 if self.device_mode else RTCC_HOST_PTRS
+        rc = lib.rtcc_create(ctypes.byref(h), oa, ob, va, vb, n_chol, _ptr(L), _ptr(fock), flags,
+                             ctypes.c_void_p(stream or 0))
+        if rc:
+            raise RtccError(rc, "rtcc_create")
+        self._h = h
+        a, b, w = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong()
+        lib.rtcc_sizes(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(w))
+        self.n_t1, self.n_t2, self.workspace_bytes = a.value, b.value, w.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.rtcc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc, what):
+        if rc:
+            raise RtccError(rc, what, self._lib.rtcc_last_cuda_error(self._h))
+
+    def _new(self, n):
+        if self.device_mode:
+            import torch
+            return torch.empty(n, dtype=torch.complex128, device="cuda")
+        return np.empty(n, dtype=np.complex128)
+
+    def _chk(self, x, n):
+        if self.device_mode:
+            assert _is_torch(x) and x.is_cuda and x.is_contiguous() and x.numel() == n
+            return x
+        x = np.ascontiguousarray(x, dtype=np.complex128)
+        assert x.size == n
+        return x
+
+    def residual(self, t1, t2, r1=None, r2=None):
+        """R1, R2 (packed) at the given packed amplitudes; E via residual_energy()."""
+        t1 = self._chk(t1, self.n_t1); t2 = self._chk(t2, self.n_t2)
+        r1 = self._new(self.n_t1) if r1 is None else r1
+        r2 = self._new(self.n_t2) if r2 is None else r2
+        self._ck(self._lib.rtcc_residual(self._h, _ptr(t1), _ptr(t2), _ptr(r1), _ptr(r2)), "rtcc_residual")
+        return r1, r2
+
+    def residual_energy(self) -> complex:
+        out = (ctypes.c_double * 2)()
+        self._ck(self._lib.rtcc_residual_energy(self._h, out), "rtcc_residual_energy")
+        return complex(out[0], out[1])
+
+    def set_amplitudes(self, t1, t2, time=0.0, C=0j):
+        t1 = self._chk(t1, self.n_t1); t2 = self._chk(t2, self.n_t2)
+        c = (ctypes.c_double * 2)(complex(C).real, complex(C).imag)
+        self._ck(self._lib.rtcc_set_amplitudes(self._h, _ptr(t1), _ptr(t2), float(time), c), "rtcc_set_amplitudes")
+
+    def get_amplitudes(self):
+        t1, t2 = self._new(self.n_t1), self._new(self.n_t2)
+        self._ck(self._lib.rtcc_get_amplitudes(self._h, _ptr(t1), _ptr(t2)), "rtcc_get_amplitudes")
+        return t1, t2
+
+    def set_solver(self, mode=0, tol=1e-4, max_micro=200, fixed_micro=0):
+        self._ck(self._lib.rtcc_set_solver(self._h, mode, tol, max_micro, fixed_micro), "rtcc_set_solver")
+
+    def step(self, dt: float) -> int:
+        self._ck(self._lib.rtcc_step(self._h, float(dt)), "rtcc_step")
+        return self._lib.rtcc_last_micro_iterations(self._h)
+
+    def cumulant(self):
+        """(C, E) at the current time."""
+        out = (ctypes.c_double * 4)()
+        self._ck(self._lib.rtcc_cumulant(self._h, out), "rtcc_cumulant")
+        return complex(out[0], out[1]), complex(out[2], out[3])
+
+    @property
+    def time(self) -> float:
+        return self._lib.rtcc_time(self._h)
+
+    def counters(self):
+        a, f = ctypes.c_longlong(), ctypes.c_double()
+        self._ck(self._lib.rtcc_counters(self._h, ctypes.byref(a), ctypes.byref(f)), "rtcc_counters")
+        return a.value, f.value
+
+    def reset_counters(self):
+        self._ck(self._lib.rtcc_reset_counters(self._h), "rtcc_reset_counters")
+
+    def set_timing(self, on: bool):
+        self._ck(self._lib.rtcc_set_timing(self._h, int(on)), "rtcc_set_timing")
+
+    def ladder_timing(self):
+        """(ms, executed flops, model flops) of the pp-ladder kernels of the last timed residual."""
+        a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        self._ck(self._lib.rtcc_ladder_timing(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "rtcc_ladder_timing")
+        return a.value, b.value, c.value
+
+    def debug_buffer(self, name: str) -> np.ndarray:
+        n = self._lib.rtcc_debug_buffer(self._h, name.encode(), None, 0)
+        if n < 0:
+            raise RtccError(int(n), f"rtcc_debug_buffer({name})")
+        out = np.empty(n, dtype=np.float64)
+        self._lib.rtcc_debug_buffer(self._h, name.encode(), _ptr(out), n)
+        return out
