@@ -14,6 +14,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 namespace rtcc {
 
@@ -277,7 +278,13 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     if (g.Klo <= 0 || g.Klo >= g.K) g.Klo = 0x40000000;
     const int nbt = g.nb * g.nsb;
     const long long t128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * nbt;
-    const bool big = t128 >= (long long)(num_sms * 3) / 4 && g.M > 64 && g.N > 64;
+    bool big = t128 >= (long long)(num_sms * 3) / 4 && g.M > 64 && g.N > 64;
+    {   // debugging override: RTCC_TILE=64 / 128 forces a tile configuration
+        static int forced = -1;
+        if (forced < 0) { const char* e = getenv("RTCC_TILE"); forced = e ? atoi(e) : 0; }
+        if (forced == 64) big = false;
+        if (forced == 128) big = true;
+    }
     const int BM = big ? 128 : 64, BN = big ? 128 : 64;
     const long long tiles = (long long)((g.M + BM - 1) / BM) * ((g.N + BN - 1) / BN) * nbt;
     const int nkt = (g.K + 15) / 16;
