@@ -35,6 +35,7 @@ struct rtcc_ctx {
     double *Xss[2]{}, *tauss[2]{}, *Yss[2]{}, *W4[2]{}, *Wp[2]{}, *Yoop[2]{}, *Zv[2]{};
     int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
     int ntiles_ab = 0, ntiles_ss[2]{};
+    LadderBatch lb{};
     double* ws = nullptr; long long ws_cap = 0;
     double *partial = nullptr, *bmax = nullptr, *scal = nullptr;   // scal: [0..1] E, [2] delta
     double* h_scal = nullptr;                                      // pinned host mirror of scal
@@ -410,27 +411,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 11. ladders (pp with all-orbital rows; hh and the T1 corrections from the occupied rows)
-    if (c->timing && !c->capturing) { CK(cudaEventRecord(c->ev[0], st)); c->lad_flops = 0.0; }
-    double* lf = (c->timing && !c->capturing) ? &c->lad_flops : nullptr;
-    if (d.oo > 0) {
-        LadderArgs a;
-        a.LA = c->L[0]; a.LB = c->L[1]; a.sQA = a.sQB = nn; a.ldA = a.ldB = n; a.offA = d.o[0]; a.offB = d.o[1];
-        a.nA = a.nB = n; a.vA = d.v[0]; a.vB = d.v[1]; a.NQ = NQ;
-        a.X = c->Xab; a.ldX = 2LL * d.oo; a.N2 = 2 * d.oo; a.Y = c->Yab; a.ldY = 2LL * d.oo;
-        a.tiles = c->tiles_ab; a.ntiles = c->ntiles_ab;
-        c->launches += ladder_launch(a, st, &c->flops);
-        if (lf) ladder_launch_flops(a, lf);
-    }
-    for (int s = 0; s < 2; ++s) {
-        if (d.po[s] == 0) continue;
-        LadderArgs a;
-        a.LA = a.LB = c->L[s]; a.sQA = a.sQB = nn; a.ldA = a.ldB = n; a.offA = a.offB = d.o[s];
-        a.nA = a.nB = n; a.vA = a.vB = d.v[s]; a.NQ = NQ;
-        a.X = c->Xss[s]; a.ldX = 2LL * d.po[s]; a.N2 = 2 * d.po[s]; a.Y = c->Yss[s]; a.ldY = 2LL * d.po[s];
-        a.tiles = c->tiles_ss[s]; a.ntiles = c->ntiles_ss[s];
-        c->launches += ladder_launch(a, st, &c->flops);
-        if (lf) ladder_launch_flops(a, lf);
-    }
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], st));
+    c->launches += ladder_launch(c->lb, st, c->num_sms);
+    c->flops += ladder_flops(c->lb);
+    c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], st));
 
     if (d.oo > 0) {
@@ -737,6 +721,28 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 CKC(cudaMemcpy(c->tiles_ss[s], tss.data(), tss.size() * sizeof(int2), cudaMemcpyHostToDevice));
                 c->ntiles_ss[s] = (int)tss.size();
             }
+        }
+        {   // ladder work plan: one launch for the ab, aa, bb cases
+            LadderBatch& B = c->lb;
+            B.ncase = 0; B.NQ = NQ;
+            auto add = [&](int sa, int sb, const double* X, int cols, double* Y, const int2* tiles, int ntiles) {
+                if (cols <= 0 || ntiles <= 0) return;
+                LadderCase& g = B.c[B.ncase++];
+                g.LA = c->L[sa]; g.LB = c->L[sb]; g.sQA = g.sQB = nn; g.ldA = g.ldB = n; g.offA = d.o[sa]; g.offB = d.o[sb];
+                g.nA = g.nB = n; g.vA = d.v[sa]; g.vB = d.v[sb];
+                g.X = X; g.ldX = 2LL * cols; g.N2 = 2 * cols; g.Y = Y; g.ldY = 2LL * cols; g.Ypart = nullptr;
+                g.tiles = tiles; g.ntiles = ntiles;
+            };
+            add(0, 1, c->Xab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
+            add(0, 0, c->Xss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
+            add(1, 1, c->Xss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
+            ladder_plan(B, c->num_sms, 8);
+            for (int i = 0; i < B.ncase; ++i)
+                if (B.c[i].nsplit > 1) {
+                    const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;
+                    DA(B.c[i].Ypart, cnt, nullptr);
+                    CKC(cudaMemsetAsync(B.c[i].Ypart, 0, (size_t)cnt * 8, c->st));
+                }
         }
         // constant integral blocks: Kx (exchange-type oovv), K_bare added to the Fock matrix
         for (int s = 0; s < 2; ++s) {
