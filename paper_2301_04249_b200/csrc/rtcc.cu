@@ -21,6 +21,10 @@ struct rtcc_ctx {
     Dims d{};
     unsigned flags = 0;
     cudaStream_t st = nullptr;
+    cudaStream_t S[4]{};                 // S[0] = st (or the capture stream), S[1..3] = helper branches
+    cudaStream_t aux[3]{};
+    cudaEvent_t evs[8]{};
+    int si = 0;
     int num_sms = 148;
     int cuda_err = 0;
     std::vector<void*> allocs;
@@ -104,12 +108,13 @@ void ops_cc(TcGemm& g, const double* A, long long pA, const double* B, long long
 }
 void run(rtcc_ctx* c, TcGemm& g)
 {
-    g.ws = c->ws;
-    int n = tcgemm_launch(g, c->st, c->ws_cap, c->num_sms, &c->flops);
+    const long long cap = c->ws_cap / 4;
+    g.ws = c->ws + c->si * cap;
+    int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops);
     c->launches += n;
 }
 inline int nblk(long long n, int cap) { long long b = (n + 255) / 256; if (b < 1) b = 1; if (b > cap) b = cap; return (int)b; }
-#define EW(c, kern, n, ...) do { kern<<<nblk((n), (c)->num_sms * 16), 256, 0, (c)->st>>>(__VA_ARGS__); (c)->launches++; } while (0)
+#define EW(c, kern, n, ...) do { kern<<<nblk((n), (c)->num_sms * 16), 256, 0, (c)->S[(c)->si]>>>(__VA_ARGS__); (c)->launches++; } while (0)
 
 }  // namespace
 
@@ -126,7 +131,16 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     const long long nn = (long long)n * n, plane = (long long)NQ * nn, ld1 = 2LL * n1;
     const double* t1p = x;
     const double* t2p = x + 2 * d.n_t1;
-    cudaStream_t st = c->st;
+    // Independent parts of the evaluation run on helper streams (forked / joined with events, so the same code
+    // captures into one CUDA graph with parallel branches).  Timing mode keeps everything on one stream.
+    const bool par = !c->timing;
+    c->S[0] = c->st;
+    for (int i = 0; i < 3; ++i) c->S[i + 1] = par ? c->aux[i] : c->st;
+#define ST (c->S[c->si])
+#define BR(i) (c->si = (i))
+#define LINK(from, to, e) do { if (par) { CK(cudaEventRecord(c->evs[e], c->S[from])); CK(cudaStreamWaitEvent(c->S[to], c->evs[e], 0)); } } while (0)
+#define WAITEV(to, e) do { if (par) CK(cudaStreamWaitEvent(c->S[to], c->evs[e], 0)); } while (0)
+    BR(0);
 
     // ---- 1. unpack the packed spin blocks into the contraction layouts
     EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
@@ -137,12 +151,14 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         if (d.po[s] > 0)
             EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->tauss[s]);
 
+    if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
+
     // ---- 2. T1-dressed Cholesky vectors  L~^Q = (1-T) L^Q (1+T)
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
-        CK(cudaMemcpyAsync(c->Lt[s], c->L[s], plane * 8, cudaMemcpyDeviceToDevice, st));
-        CK(cudaMemsetAsync(c->Lt[s] + plane, 0, plane * 8, st));
+        CK(cudaMemcpyAsync(c->Lt[s], c->L[s], plane * 8, cudaMemcpyDeviceToDevice, ST));
+        CK(cudaMemsetAsync(c->Lt[s] + plane, 0, plane * 8, ST));
         if (o == 0) continue;
         {   // (L Y)[Q][p][i] += sum_e L[Q][p][o+e] t_i^e
             TcGemm g = G0(NQ * n, o, v);
@@ -163,6 +179,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             run(c, g);
         }
     }
+
+    if (par) CK(cudaEventRecord(c->evs[1], c->S[0]));     // evs[1]: dressed vectors ready
 
     // ---- 3. gamma^Q = sum_ie L^Q_ie t_i^e (both spins)
     for (int s = 0; s < 2; ++s) {
@@ -195,8 +213,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         EnergyArgs ea;
         for (int s = 0; s < 2; ++s) { ea.L[s] = c->L[s]; ea.Lt[s] = c->Lt[s]; ea.fock[s] = c->fockd[s]; }
         ea.t1r = c->t1r; ea.Mq = c->Mq; ea.gam = c->gam; ea.partial = c->partial;
-        k_energy<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d, ea);
-        k_sum_partials<<<1, 32, 0, st>>>(c->partial, RED_BLOCKS, c->scal);
+        k_energy<<<RED_BLOCKS, RED_THREADS, 0, ST>>>(d, ea);
+        k_sum_partials<<<1, 32, 0, ST>>>(c->partial, RED_BLOCKS, c->scal);
         c->launches += 2;
     }
 
@@ -205,8 +223,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
         double* F = c->Ft[s];
-        CK(cudaMemcpyAsync(F, c->Fb[s], nn * 8, cudaMemcpyDeviceToDevice, st));
-        CK(cudaMemsetAsync(F + nn, 0, nn * 8, st));
+        CK(cudaMemcpyAsync(F, c->Fb[s], nn * 8, cudaMemcpyDeviceToDevice, ST));
+        CK(cudaMemsetAsync(F + nn, 0, nn * 8, ST));
         {
             TcGemm g = G0((int)nn, 1, NQ);
             setA(g, 0, 1, 0, 0, nn, 0, 0);
@@ -265,6 +283,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         }
     }
 
+    if (par) CK(cudaEventRecord(c->evs[2], c->S[0]));     // evs[2]: F intermediates ready
+
     // ---- 7. singles:  r1 = sum_me t_im^ae f~_me - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af   (+ f~_ai at assembly)
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
@@ -314,6 +334,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 9. exchange ring channel + F terms, spin-conserving sector:  Zsc -= T (Xd + 1/2 Kx T + Fd)
+    BR(1);
+    WAITEV(1, 1);
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s], n1s = o * v;
         const long long off1 = s ? d.n1a : 0;
@@ -336,8 +358,11 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             g.beta = 1.0;
             run(c, g);
         }
+        if (s == 0 || d.n1a == 0) WAITEV(1, 2);
         EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1);
     }
+    LINK(1, 0, 3);
+    BR(0);
     {
         TcGemm g = G0(n1, n1, n1);
         setA(g, 0, ld1, 0, 0, 1, 0, 1);
@@ -349,6 +374,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 10. spin-flip sector
+    BR(2);
+    WAITEV(2, 1);
     if (d.nA > 0 && d.nB > 0) {
         const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], nA = d.nA, nB = d.nB;
         const long long lA = 2LL * nA, lB = 2LL * nB;
@@ -370,6 +397,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             g.beta = 1.0;
             run(c, g);
         }
+        WAITEV(2, 2);
         EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL);
         {
             TcGemm g = G0(nA, nB, nB);
@@ -411,11 +439,14 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 11. ladders (pp with all-orbital rows; hh and the T1 corrections from the occupied rows)
-    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], st));
-    c->launches += ladder_launch(c->lb, st, c->num_sms);
+    BR(3);
+    WAITEV(3, 0);
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
+    c->launches += ladder_launch(c->lb, ST, c->num_sms);
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
-    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], st));
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], ST));
+    WAITEV(3, 1);
 
     if (d.oo > 0) {
         const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], oo = d.oo;
@@ -510,6 +541,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         }
     }
 
+    LINK(2, 0, 4);
+    LINK(3, 0, 5);
+    BR(0);
+
     // ---- 12. antisymmetrise and write the packed residual
     {
         AsmArgs A;
@@ -599,6 +634,8 @@ void rtcc_destroy(rtcc_ctx* c)
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->ev[0]) cudaEventDestroy(c->ev[0]);
     if (c->ev[1]) cudaEventDestroy(c->ev[1]);
+    for (int i = 0; i < 3; ++i) if (c->aux[i]) cudaStreamDestroy(c->aux[i]);
+    for (int i = 0; i < 8; ++i) if (c->evs[i]) cudaEventDestroy(c->evs[i]);
     for (void* p : c->allocs) cudaFree(p);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -642,6 +679,9 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(ladder_init());
         CKC(cudaEventCreate(&c->ev[0]));
         CKC(cudaEventCreate(&c->ev[1]));
+        for (int i = 0; i < 3; ++i) CKC(cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 8; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
+        c->S[0] = c->S[1] = c->S[2] = c->S[3] = c->st; c->si = 0;
         CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
 
         for (int s = 0; s < 2; ++s) {
@@ -678,7 +718,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
         DA(c->Yab, nn * 2 * d.oo, "Yab");
         DA(c->Wooab, (long long)d.oo * 2 * d.oo, nullptr);
-        c->ws_cap = 8LL << 20;
+        c->ws_cap = 16LL << 20;
         DA(c->ws, c->ws_cap, nullptr);
         DA(c->partial, 2 * RED_BLOCKS, nullptr);
         DA(c->bmax, RED_BLOCKS, nullptr);
