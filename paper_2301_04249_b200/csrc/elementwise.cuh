@@ -45,6 +45,26 @@ __device__ __forceinline__ c128 ab_amp(const double* t2p, const Dims& d, int i, 
     return z;
 }
 
+// tile-major zero-padded slabs of the bare vectors for the ladder's bulk copies (see ladder.cuh):
+//   rows of PR orbitals x PC virtual columns, pitch PR*PC+4:  T[pt][ct][Qt][16 k][pi*PC + ci]
+__global__ void k_tile_L(int NQ, int n, int o, int v, int PR, int PC, int nCt, int nQt, const double* __restrict__ L, double* __restrict__ T)
+{
+    const long long tot = (long long)NQ * n * v;
+    const int pitch = PR * PC + 4;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        int ee = (int)(x % v); long long r = x / v; int p = (int)(r % n); int Q = (int)(r / n);
+        long long blk = ((long long)(p / PR) * nCt + ee / PC) * nQt + Q / 16;
+        T[(blk * 16 + Q % 16) * pitch + (p % PR) * PC + ee % PC] = L[((long long)Q * n + p) * n + o + ee];
+    }
+}
+// index of amplitude (e, f, col) in the ladder's tile-major X: Xt[et][ft][ct][8 kt][16][nt2+4]
+__device__ __forceinline__ long long xt_index(int e, int f, int col, int nFt, int ncol, int nt2)
+{
+    const int k2 = (e % 16) * 8 + (f % 8);
+    long long t = (((long long)(e / 16) * nFt + f / 8) * ncol + col / nt2) * 8 + k2 / 16;
+    return (t * 16 + k2 % 16) * (nt2 + 4) + col % nt2;
+}
+
 // t1 packed -> planar t1r[pl][x], x in sc pair order (alpha (i,a) then beta)
 __global__ void k_unpack_t1(Dims d, const double* __restrict__ t1p, double* __restrict__ t1r)
 {
@@ -89,7 +109,7 @@ __global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __re
 
 // X_ab[(e,F)][pl][(i,J)] = tab[i,J,e,F];  tau_ab = X + t1a[i,e] t1b[J,F]
 __global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double* __restrict__ t1r,
-                            double* __restrict__ X, double* __restrict__ tau)
+                            double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau)
 {
     const long long tot = (long long)d.v[0] * d.v[1] * d.oo;
     for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
@@ -101,6 +121,8 @@ __global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double
         double ar = t1r[xa], ai = t1r[d.n1 + xa], br = t1r[xb], bi = t1r[d.n1 + xb];
         X[row * 2 * d.oo + col] = z.re;
         X[row * 2 * d.oo + d.oo + col] = z.im;
+        Xt[xt_index(e, F, col, nFt, ncol, nt2)] = z.re;
+        Xt[xt_index(e, F, d.oo + col, nFt, ncol, nt2)] = z.im;
         tau[row * 2 * d.oo + col] = z.re + ar * br - ai * bi;
         tau[row * 2 * d.oo + d.oo + col] = z.im + ar * bi + ai * br;
     }
@@ -108,7 +130,7 @@ __global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double
 
 // X_ss[(e,f)][pl][(i<j)] = t_{ij}^{ef};  tau = X + t1[i,e] t1[j,f] - t1[i,f] t1[j,e]
 __global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const double* __restrict__ t1r,
-                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ tau)
+                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau)
 {
     const int v = d.v[s], po = d.po[s];
     const long long tot = (long long)v * v * po;
@@ -124,6 +146,8 @@ __global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const
         double ti = t1r[ie] * t1r[d.n1 + jf] + t1r[d.n1 + ie] * t1r[jf] - (t1r[iff] * t1r[d.n1 + je] + t1r[d.n1 + iff] * t1r[je]);
         X[row * 2 * po + col] = z.re;
         X[row * 2 * po + po + col] = z.im;
+        Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
+        Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;
         tau[row * 2 * po + col] = z.re + tr;
         tau[row * 2 * po + po + col] = z.im + ti;
     }

@@ -13,8 +13,9 @@
 //   GEMM-1  W[(p,e),(q,f)] = sum_Q LA^T LB          (128 x 64 x n_chol, DMMA, accumulators in registers)
 //   re-index W -> shared memory as A-operand [(p,q)][(e,f)]   (64 x 128)
 //   GEMM-2  acc[(p,q)][x] += W * X[(e,f) chunk][x]  (64 x NT2 x 128, DMMA)
-// Both GEMMs stream their global operands through one 3-stage cp.async pipeline whose producer keeps
-// running pointers (no divisions, no 64-bit multiplies in the steady state).  When the (e,f) plane is
+// Both GEMMs stream their global operands through one 4-stage ring filled by a dedicated producer warp with
+// 1-D bulk async copies (cp.async.bulk, TMA engine) from zero-padded operand slabs, completion tracked by
+// mbarriers; the 8 consumer warps execute only LDS + DMMA.  When the (e,f) plane is
 // sliced (small problems: more items than SMs), each slice writes its own partial buffer and
 // ladder_reduce_kernel sums them in a fixed order -- no atomics, bit-reproducible.
 #pragma once
@@ -23,13 +24,14 @@
 namespace rtcc {
 
 struct LadderCase {
-    const double* LA; const double* LB;   // bare Cholesky vectors of the two spins, [NQ][n][n]
-    long long sQA, sQB;                   // stride between Cholesky vectors
-    int ldA, ldB;                         // row pitch (orbital count n)
-    int offA, offB;                       // first virtual column (o_sigma)
-    int nA, nB;                           // number of rows p / q
-    int vA, vB;                           // number of virtuals e / f
-    const double* X; long long ldX;       // [(e*vB+f)][N2]
+    // Tile-major, zero-padded slabs of the bare Cholesky vectors' virtual columns, laid out exactly as the
+    // shared-memory stage wants them (row pitch == 4 mod 16 doubles), so that each pipeline tile is ONE bulk copy:
+    //   LA[pt][et][Qt][16 k][8 p x 16 e (+4 pad)]      LB[qt][ft][Qt][16 k][8 q x 8 f (+4 pad)]
+    const double* LA; const double* LB;
+    int nA, nB;                           // number of rows p / q (unpadded)
+    int vA, vB;                           // number of virtuals e / f (unpadded)
+    // amplitudes, tile-major and zero padded: Xt[et][ft][ct][8 kt][16 rows (e_in*8+f_in)][nt2 (+4 pad)]
+    const double* X;
     int N2;
     double* Y; long long ldY;             // [(p*nB+q)][N2]
     double* Ypart;                        // [nsplit][nA*nB][ldY] when nsplit > 1
@@ -41,7 +43,7 @@ struct LadderCase {
 };
 struct LadderBatch {
     LadderCase c[3];
-    int ncase, NQ, nitems;
+    int ncase, NQ, nitems;                // NQ: padded to a multiple of 16
 };
 
 constexpr int LD_PP = 8, LD_PQ = 8, LD_PE = 16, LD_PF = 8;
@@ -49,104 +51,101 @@ constexpr int LD_M1 = LD_PP * LD_PE;      // 128
 constexpr int LD_N1 = LD_PQ * LD_PF;      // 64
 constexpr int LD_R = LD_PP * LD_PQ;       // 64 rows
 constexpr int LD_K2 = LD_PE * LD_PF;      // 128
-constexpr int LD_BK = 16, LD_ST = 3;
+constexpr int LD_BK = 16, LD_ST = 4;
 constexpr int LD_LDA1 = LD_M1 + 4, LD_LDB1 = LD_N1 + 4, LD_LDW = LD_K2 + 4;
 constexpr int LD_STAGE = LD_BK * (LD_LDA1 + LD_LDB1);      // >= 16*(128+4)
+constexpr int LD_NCONS = 256, LD_NTH = 288;               // 8 consumer warps + 1 producer warp
 
-constexpr size_t ladder_smem() { return sizeof(double) * (LD_ST * (size_t)LD_STAGE + (size_t)LD_R * LD_LDW); }
+constexpr size_t ladder_smem() { return sizeof(double) * (LD_ST * (size_t)LD_STAGE + (size_t)LD_R * LD_LDW) + 2 * LD_ST * sizeof(unsigned long long); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count)
+{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes)
+{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b)
+{ asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
+        ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+}
+// 1-D bulk async copy global -> shared (TMA engine), completion counted in bytes on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
 template <int NT2>
-__device__ __forceinline__ void ladder_body(const LadderCase& g, const int NQ, const int p0, const int q0, const int x0,
+__device__ __forceinline__ void ladder_body(const LadderCase& gc, const int NQ, const int p0, const int q0, const int x0,
                                             const int ch_begin, const int ch_end, double* __restrict__ Yout, double* smem)
 {
-    constexpr int NTH = 256;
     constexpr int LDX2 = NT2 + 4;
     constexpr int WGN = NT2 / 32;               // GEMM-2 warp grid: (8/WGN) x WGN, warp tile WM2 x 32
     constexpr int WGM = 8 / WGN;
     constexpr int WM2 = LD_R / WGM;             // 32 (NT2=128) or 16 (NT2=64)
     constexpr int TM2 = WM2 / 8;
-    constexpr int RPP = NTH / NT2;              // X rows per pass: 2 or 4
     double* stg = smem;
     double* Ws = smem + LD_ST * LD_STAGE;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(Ws + LD_R * LD_LDW);
+    unsigned long long* empty = full + LD_ST;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int lr = lane >> 2, lc = lane & 3;
-    const int nFt = (g.vB + LD_PF - 1) / LD_PF;
-    const int T1 = (NQ + LD_BK - 1) / LD_BK;
+    const int nFt = (gc.vB + LD_PF - 1) / LD_PF;
+    const int T1 = NQ / LD_BK;
     constexpr int T2 = LD_K2 / LD_BK;
     const int tpc = T1 + T2;
     const int total = (ch_end - ch_begin) * tpc;
 
-    // ---- producer state (running pointers)
-    const int mA = tid % LD_M1, kA0 = tid / LD_M1;           // A1: 2 k-rows per pass, 8 passes
-    const int nB = tid % LD_N1, kB0 = tid / LD_N1;           // B1: 4 k-rows per pass, 4 passes
-    const int pA = mA / LD_PE, eA = mA % LD_PE, qB = nB / LD_PF, fB = nB % LD_PF;
-    const bool rowA = p0 + pA < g.nA, rowB = q0 + qB < g.nB;
-    const double* baseA = g.LA + (long long)(p0 + pA) * g.ldA + g.offA + eA + kA0 * g.sQA;
-    const double* baseB = g.LB + (long long)(q0 + qB) * g.ldB + g.offB + fB + kB0 * g.sQB;
-    const long long stepA = 2 * g.sQA, stepB = 4 * g.sQB;
-    const int cX = tid % NT2, kX0 = tid / NT2;
-    const bool colX = x0 + cX < g.N2;
-    const long long sF = g.ldX, sE = g.ldX * g.vB;
-    const double* baseX = g.X + x0 + cX;
-    int p_ch = ch_begin, p_r = 0;
-    int p_e0 = (ch_begin / nFt) * LD_PE, p_f0 = (ch_begin % nFt) * LD_PF;
-    const double* curA = baseA + p_e0;
-    const double* curB = baseB + p_f0;
+    if (tid == 0) {
+        for (int s = 0; s < LD_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
 
-    auto produce = [&](int stage) {
-        double* sb = stg + stage * LD_STAGE;
-        if (p_r < T1) {
-            const int kb = p_r * LD_BK;
-            {
-                const bool mv = rowA && (p_e0 + eA < g.vA);
-                const double* s = curA;
-                double* d = sb + kA0 * LD_LDA1 + mA;
-#pragma unroll
-                for (int j = 0; j < LD_BK / 2; ++j) {
-                    const bool v = mv && (kb + kA0 + 2 * j < NQ);
-                    cp_async8(d + 2 * j * LD_LDA1, v ? s : g.LA, v);
-                    s += stepA;
+    if (warp == 8) {
+        // ---------------- producer: one elected lane, one or two bulk copies per tile
+        if (lane == 0) {
+            const int nEt = (gc.vA + LD_PE - 1) / LD_PE;
+            constexpr int BLKA = LD_BK * LD_LDA1, BLKB = LD_BK * LD_LDB1, BLKX = LD_BK * LDX2;
+            const int ncol = gc.ncol, ct = x0 / NT2;
+            const double* LAp = gc.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA;
+            const double* LBp = gc.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB;
+            int et = ch_begin / nFt, ft = ch_begin % nFt, r = 0;
+            const double* curA = LAp + (long long)et * T1 * BLKA;
+            const double* curB = LBp + (long long)ft * T1 * BLKB;
+            const double* curX = gc.X + (((long long)(et * nFt + ft) * ncol + ct) * T2) * BLKX;
+            int stage = 0; unsigned par = 1;       // first pass over the ring: slots are free
+            for (int it = 0; it < total; ++it) {
+                mbar_wait(&empty[stage], par);
+                double* sb = stg + stage * LD_STAGE;
+                if (r < T1) {
+                    mbar_expect_tx(&full[stage], (BLKA + BLKB) * 8);
+                    bulk_g2s(sb, curA, BLKA * 8, &full[stage]);
+                    bulk_g2s(sb + BLKA, curB, BLKB * 8, &full[stage]);
+                    curA += BLKA; curB += BLKB;
+                } else {
+                    mbar_expect_tx(&full[stage], BLKX * 8);
+                    bulk_g2s(sb, curX, BLKX * 8, &full[stage]);
+                    curX += BLKX;
                 }
-                curA = s;
-            }
-            {
-                const bool nv = rowB && (p_f0 + fB < g.vB);
-                const double* s = curB;
-                double* d = sb + LD_BK * LD_LDA1 + kB0 * LD_LDB1 + nB;
-#pragma unroll
-                for (int j = 0; j < LD_BK / 4; ++j) {
-                    const bool v = nv && (kb + kB0 + 4 * j < NQ);
-                    cp_async8(d + 4 * j * LD_LDB1, v ? s : g.LB, v);
-                    s += stepB;
+                if (++r == tpc) {
+                    r = 0;
+                    if (++ft == nFt) { ft = 0; ++et; }
+                    curA = LAp + (long long)et * T1 * BLKA;
+                    curB = LBp + (long long)ft * T1 * BLKB;
+                    curX = gc.X + (((long long)(et * nFt + ft) * ncol + ct) * T2) * BLKX;
                 }
-                curB = s;
-            }
-        } else {
-            // rows kb..kb+15 of the chunk = (e, f) with e = e0 + kb/8 + {0,1}, f = f0 + 0..7
-            const int kb = (p_r - T1) * LD_BK;
-            const int eb = p_e0 + (kb >> 3);
-            const double* P0 = baseX + ((long long)eb * g.vB + p_f0) * g.ldX;
-            double* d = sb + kX0 * LDX2 + cX;
-#pragma unroll
-            for (int j = 0; j < LD_BK / RPP; ++j) {
-                const int kk = kX0 + RPP * j;                 // compile-time pattern: kk>>3, kk&7
-                const int de = (RPP * j + (RPP - 1)) >> 3;    // same for every kX0 < RPP because RPP divides 8
-                const int ff = kk & 7;
-                const bool v = colX && (eb + de < g.vA) && (p_f0 + ff < g.vB);
-                const double* s = P0 + de * sE + ff * sF;
-                cp_async8(d + RPP * j * LDX2, v ? s : g.X, v);
+                if (++stage == LD_ST) { stage = 0; par ^= 1; }
             }
         }
-        if (++p_r == tpc) {
-            p_r = 0; ++p_ch;
-            p_f0 += LD_PF;
-            if (p_f0 >= nFt * LD_PF) { p_f0 = 0; p_e0 += LD_PE; }
-            curA = baseA + p_e0;
-            curB = baseB + p_f0;
-        }
-    };
+        return;
+    }
 
+    // ---------------- consumer warps
+    const int lr = lane >> 2, lc = lane & 3;
     double acc2[TM2][4][2];
 #pragma unroll
     for (int i = 0; i < TM2; ++i)
@@ -158,21 +157,10 @@ __device__ __forceinline__ void ladder_body(const LadderCase& g, const int NQ, c
     const int w1m = (warp >> 1) * 32, w1n = (warp & 1) * 32;
     const int w2m = (warp / WGN) * WM2, w2n = (warp % WGN) * 32;
 
-    int issued = 0;
-#pragma unroll
-    for (int s = 0; s < LD_ST - 1; ++s) {
-        if (issued < total) { produce(s); ++issued; }
-        cp_async_commit();
-    }
-    int r = 0, cstage = 0, pstage = LD_ST - 1;
-    for (int s = 0; s < total; ++s) {
-        cp_async_wait<LD_ST - 2>();
-        __syncthreads();
-        if (issued < total) { produce(pstage); ++issued; }
-        cp_async_commit();
-        if (++pstage == LD_ST) pstage = 0;
-        const double* sb = stg + cstage * LD_STAGE;
-        if (++cstage == LD_ST) cstage = 0;
+    int r = 0, stage = 0; unsigned par = 0;
+    for (int it = 0; it < total; ++it) {
+        mbar_wait(&full[stage], par);
+        const double* sb = stg + stage * LD_STAGE;
         if (r < T1) {
             if (r == 0) {
 #pragma unroll
@@ -194,9 +182,10 @@ __device__ __forceinline__ void ladder_body(const LadderCase& g, const int NQ, c
 #pragma unroll
                     for (int j = 0; j < 4; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], a[i], b[j]);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[stage]);
             if (r == T1 - 1) {
-                // W[(p,e),(q,f)] -> Ws[(p,q)][(e,f)].  The previous chunk's GEMM-2 finished reading Ws
-                // at least one __syncthreads ago (T1 >= 1 tiles of GEMM-1 lie in between).
+                bar_consumers();        // every consumer has finished the previous chunk's GEMM-2 reads of Ws
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     const int m = w1m + 8 * i + lr;
@@ -209,6 +198,7 @@ __device__ __forceinline__ void ladder_body(const LadderCase& g, const int NQ, c
                             make_double2(acc1[i][j][0], acc1[i][j][1]);
                     }
                 }
+                bar_consumers();        // W chunk complete
             }
         } else {
             const int kb = (r - T1) * LD_BK;
@@ -226,30 +216,32 @@ __device__ __forceinline__ void ladder_body(const LadderCase& g, const int NQ, c
 #pragma unroll
                     for (int j = 0; j < 4; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], a[i], b[j]);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[stage]);
         }
         if (++r == tpc) r = 0;
+        if (++stage == LD_ST) { stage = 0; par ^= 1; }
     }
-    cp_async_wait<0>();
 
 #pragma unroll
     for (int i = 0; i < TM2; ++i) {
         const int row = w2m + 8 * i + lr;
         const int p = p0 + row / LD_PQ, q = q0 + row % LD_PQ;
-        if (p >= g.nA || q >= g.nB) continue;
-        double* y = Yout + ((long long)p * g.nB + q) * g.ldY;
+        if (p >= gc.nA || q >= gc.nB) continue;
+        double* y = Yout + ((long long)p * gc.nB + q) * gc.ldY;
 #pragma unroll
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
                 const int x = x0 + w2n + 8 * j + 2 * lc + c;
-                if (x < g.N2) y[x] = acc2[i][j][c];
+                if (x < gc.N2) y[x] = acc2[i][j][c];
             }
     }
 }
 
-__global__ void __launch_bounds__(256) ladder_kernel(const LadderBatch b)
+__global__ void __launch_bounds__(LD_NTH) ladder_kernel(const LadderBatch b)
 {
-    extern __shared__ double smem[];
+    extern __shared__ __align__(128) double smem[];
     int item = blockIdx.x, ci = 0;
     if (b.ncase > 1 && item >= b.c[1].item0) ci = 1;
     if (b.ncase > 2 && item >= b.c[2].item0) ci = 2;
@@ -327,7 +319,7 @@ inline double ladder_flops(const LadderBatch& b)
 inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
 {
     if (b.nitems <= 0) return 0;
-    ladder_kernel<<<b.nitems, 256, ladder_smem(), st>>>(b);
+    ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(b);
     bool red = false;
     for (int i = 0; i < b.ncase; ++i) red |= b.c[i].nsplit > 1;
     if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); return 2; }

@@ -36,6 +36,8 @@ struct rtcc_ctx {
     double *TAB = nullptr, *WBB = nullptr, *WAA = nullptr, *ZAB = nullptr, *ZBA = nullptr;
     double *Mq = nullptr, *gam = nullptr, *r1buf = nullptr;
     double *Xab = nullptr, *tauab = nullptr, *Yab = nullptr, *Wooab = nullptr;
+    double *LtA[2]{}, *LtB[2]{}, *Xt_ab = nullptr, *Xt_ss[2]{};   // tile-major ladder operands
+    int nt2_ab = 128, nt2_ss[2]{128, 128};
     double *Xss[2]{}, *tauss[2]{}, *Yss[2]{}, *W4[2]{}, *Wp[2]{}, *Yoop[2]{}, *Zv[2]{};
     int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
     int ntiles_ab = 0, ntiles_ss[2]{};
@@ -146,10 +148,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
     EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc);
     EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB);
-    EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->tauab);
+    EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
     for (int s = 0; s < 2; ++s)
         if (d.po[s] > 0)
-            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->tauss[s]);
+            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->Xt_ss[s], (d.v[s] + 7) / 8, (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->tauss[s]);
 
     if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
 
@@ -693,6 +695,20 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             DA(c->Kx[s], (long long)d.o[s] * d.v[s] * d.o[s] * d.v[s], s ? "Kx1" : "Kx0");
             const int po = d.po[s], v = d.v[s], o = d.o[s];
             DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
+            {
+                const int nt2 = 2 * po <= 64 ? 64 : 128;
+                c->nt2_ss[s] = nt2;
+                const long long ncol = (2 * po + nt2 - 1) / nt2;
+                const long long cx = (long long)((v + 15) / 16) * ((v + 7) / 8) * ncol * 128 * (nt2 + 4);
+                DA(c->Xt_ss[s], cx, nullptr);
+                CKC(cudaMemsetAsync(c->Xt_ss[s], 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+                const long long nQt = (NQ + 15) / 16, nPt = (n + 7) / 8;
+                const long long ca = nPt * ((v + 15) / 16) * nQt * 16 * LD_LDA1, cb = nPt * ((v + 7) / 8) * nQt * 16 * LD_LDB1;
+                DA(c->LtA[s], ca, nullptr);
+                DA(c->LtB[s], cb, nullptr);
+                CKC(cudaMemsetAsync(c->LtA[s], 0, (size_t)ca * 8, c->st));
+                CKC(cudaMemsetAsync(c->LtB[s], 0, (size_t)cb * 8, c->st));
+            }
             DA(c->tauss[s], (long long)v * v * 2 * po, nullptr);
             DA(c->Yss[s], nn * 2 * po, s ? "Yss1" : "Yss0");
             DA(c->W4[s], (long long)o * o * 2 * o * o, nullptr);
@@ -715,6 +731,14 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->gam, 2LL * NQ, "gam");
         DA(c->r1buf, 2LL * n1, "r1buf");
         DA(c->Xab, (long long)va * vb * 2 * d.oo, "Xab");
+        {
+            const int nt2 = 2 * d.oo <= 64 ? 64 : 128;
+            c->nt2_ab = nt2;
+            const long long ncol = (2 * d.oo + nt2 - 1) / nt2;
+            const long long cx = (long long)((va + 15) / 16) * ((vb + 7) / 8) * ncol * 128 * (nt2 + 4);
+            DA(c->Xt_ab, cx, nullptr);
+            CKC(cudaMemsetAsync(c->Xt_ab, 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+        }
         DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
         DA(c->Yab, nn * 2 * d.oo, "Yab");
         DA(c->Wooab, (long long)d.oo * 2 * d.oo, nullptr);
@@ -764,18 +788,24 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         }
         {   // ladder work plan: one launch for the ab, aa, bb cases
             LadderBatch& B = c->lb;
-            B.ncase = 0; B.NQ = NQ;
-            auto add = [&](int sa, int sb, const double* X, int cols, double* Y, const int2* tiles, int ntiles) {
+            B.ncase = 0;
+            B.NQ = (NQ + 15) / 16 * 16;
+            for (int s = 0; s < 2; ++s) {
+                const int v = d.v[s], nQt = (NQ + 15) / 16;
+                EW(c, k_tile_L, (long long)NQ * n * v, NQ, n, d.o[s], v, LD_PP, LD_PE, (v + 15) / 16, nQt, c->L[s], c->LtA[s]);
+                EW(c, k_tile_L, (long long)NQ * n * v, NQ, n, d.o[s], v, LD_PQ, LD_PF, (v + 7) / 8, nQt, c->L[s], c->LtB[s]);
+            }
+            auto add = [&](int sa, int sb, const double* Xt, int cols, double* Y, const int2* tiles, int ntiles) {
                 if (cols <= 0 || ntiles <= 0) return;
                 LadderCase& g = B.c[B.ncase++];
-                g.LA = c->L[sa]; g.LB = c->L[sb]; g.sQA = g.sQB = nn; g.ldA = g.ldB = n; g.offA = d.o[sa]; g.offB = d.o[sb];
+                g.LA = c->LtA[sa]; g.LB = c->LtB[sb];
                 g.nA = g.nB = n; g.vA = d.v[sa]; g.vB = d.v[sb];
-                g.X = X; g.ldX = 2LL * cols; g.N2 = 2 * cols; g.Y = Y; g.ldY = 2LL * cols; g.Ypart = nullptr;
+                g.X = Xt; g.N2 = 2 * cols; g.Y = Y; g.ldY = 2LL * cols; g.Ypart = nullptr;
                 g.tiles = tiles; g.ntiles = ntiles;
             };
-            add(0, 1, c->Xab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
-            add(0, 0, c->Xss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
-            add(1, 1, c->Xss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
+            add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
+            add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
+            add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
             ladder_plan(B, c->num_sms, 8);
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
