@@ -58,18 +58,6 @@ constexpr int LD_NCONS = 256, LD_NTH = 288;               // 8 consumer warps + 
 
 constexpr size_t ladder_smem() { return sizeof(double) * (LD_ST * (size_t)LD_STAGE + (size_t)LD_R * LD_LDW) + 2 * LD_ST * sizeof(unsigned long long); }
 
-__device__ __forceinline__ void mbar_init(unsigned long long* b, int count)
-{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count)); }
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes)
-{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(bytes) : "memory"); }
-__device__ __forceinline__ void mbar_arrive(unsigned long long* b)
-{ asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity)
-{
-    asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
-        ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
-}
 // 1-D bulk async copy global -> shared (TMA engine), completion counted in bytes on an mbarrier
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
 {

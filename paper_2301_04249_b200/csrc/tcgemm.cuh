@@ -61,19 +61,48 @@ __device__ __forceinline__ long long idx2(int x, int lo, long long s_hi, long lo
     return (long long)h * s_hi + (long long)(x - h * lo) * s_lo;
 }
 
-template <int BM, int BN, int WM, int WN>
-__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32) tcgemm_kernel(const TcGemm g)
+// ---- mbarrier / async-copy helpers (shared with ladder.cuh)
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count)
+{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes)
+{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b)
+{ asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity)
 {
-    constexpr int BK = 16, ST = 3;
-    constexpr int NTH = (BM / WM) * (BN / WN) * 32;
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
+        ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+}
+// the barrier receives one arrival when all cp.async issued so far by this thread have landed
+__device__ __forceinline__ void cp_async_mbar_arrive(unsigned long long* b)
+{ asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
+// 8-byte async copy, zero-filled when !valid (ignore-src predicate form: no size arithmetic)
+__device__ __forceinline__ void cp_async8p(void* smem_dst, const void* gsrc, bool valid)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("{\n .reg .pred p;\n setp.eq.u32 p, %2, 0;\n cp.async.ca.shared.global [%0], [%1], 8, p;\n}" ::"r"(d), "l"(gsrc), "r"((unsigned)valid) : "memory");
+}
+
+// Warp-specialised: (BM/WM)*(BN/WN) consumer warps (LDS + DMMA only) and half as many producer warps that
+// gather the tiles with 8-byte cp.async through a 4-stage mbarrier ring.
+template <int BM, int BN, int WM, int WN>
+__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(const TcGemm g)
+{
+    constexpr int BK = 16, ST = 4;
+    constexpr int NCW = (BM / WM) * (BN / WN), NPW = NCW / 2;
+    constexpr int NTH = (NCW + NPW) * 32, NP = NPW * 32;
     constexpr int LDA = BK + 4, LDB = BN + 4;
-    constexpr int EA = BM * BK / NTH, EB = BK * BN / NTH;
+    constexpr int EA = BM * BK / NP, EB = BK * BN / NP;      // 16 each
     constexpr int TM = WM / 8, TN = WN / 8;
-    extern __shared__ double smem[];
+    static_assert(NP == BM && NP == BN && EA == BK && EB == BK, "producer mapping assumes one row / column per producer thread");
+    extern __shared__ __align__(16) double smem[];
     double* As = smem;                        // [ST][BM][LDA]
     double* Bs = smem + ST * BM * LDA;        // [ST][BK][LDB]
     long long* rowA = (long long*)(Bs + ST * BK * LDB);   // [BM] offsets (or -1)
     long long* colB = rowA + BM;                          // [BN]
+    unsigned long long* full = (unsigned long long*)(colB + BN);
+    unsigned long long* empty = full + ST;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int z = blockIdx.z;
@@ -90,6 +119,10 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32) tcgemm_kernel(cons
         int n = n0 + i;
         colB[i] = (n < g.N) ? idx2(n, g.Nlo, g.bn_hi, g.bn_lo) : -1;
     }
+    if (tid == 0) {
+        for (int s = 0; s < ST; ++s) { mbar_init(&full[s], NP); mbar_init(&empty[s], NCW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     __syncthreads();
 
     const int nkt = (g.K + BK - 1) / BK;
@@ -100,66 +133,100 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32) tcgemm_kernel(cons
     const int nph = g.nphase[db];
     const int total = nk * nph;
 
-    const double* Ap[2] = {g.A[db][0] + sb * g.sbA, g.A[db][1] + sb * g.sbA};
-    const double* Bp[2] = {g.B[db][0] + sb * g.sbB, g.B[db][1] + sb * g.sbB};
-
-    auto load_tile = [&](int t, int stage) {
-        const int ph = t / nk;
-        const int kbase = (kt0 + (t - ph * nk)) * BK;
-        const double* A = Ap[ph];
-        const double* B = Bp[ph];
-        double* as = As + stage * BM * LDA;
-        double* bs = Bs + stage * BK * LDB;
-        if (g.a_kfast) {
-            const int kk = tid % BK, r0 = tid / BK;
-            const int k = kbase + kk;
-            const bool kv = k < g.K;
-            const long long ko = kv ? idx2(k, g.Klo, g.ak_hi, g.ak_lo) : 0;
+    if (warp >= NCW) {
+        // ------------------------------------------------------------ producers
+        const int p = tid - NCW * 32;
+        const double* Ap[2] = {g.A[db][0] + sb * g.sbA, g.A[db][1] + sb * g.sbA};
+        const double* Bp[2] = {g.B[db][0] + sb * g.sbB, g.B[db][1] + sb * g.sbB};
+        const bool k1 = g.Klo >= 0x40000000;            // single-level k
+        const int a_kfast = g.a_kfast, b_nfast = g.b_nfast;
+        // kfast: this thread owns k-column (p % 16) of rows p/16 + (NP/16) j;  otherwise row p, all 16 k
+        long long ra[EA];                               // row offsets (kfast) -- or ra[0] only
+        if (a_kfast) {
 #pragma unroll
-            for (int j = 0; j < EA; ++j) {
-                int r = r0 + j * (NTH / BK);
-                long long ro = rowA[r];
-                bool v = kv && ro >= 0;
-                cp_async8(as + r * LDA + kk, v ? (A + ro + ko) : A, v);
-            }
-        } else {
-            const int r = tid % BM, k0 = tid / BM;
-            const long long ro = rowA[r];
+            for (int j = 0; j < EA; ++j) ra[j] = rowA[p / BK + (NP / BK) * j];
+        } else ra[0] = rowA[p];
+        long long cb[EB];
+        if (!b_nfast) {
 #pragma unroll
-            for (int j = 0; j < EA; ++j) {
-                int kk = k0 + j * (NTH / BM);
-                int k = kbase + kk;
-                bool v = (k < g.K) && ro >= 0;
-                long long ko = v ? idx2(k, g.Klo, g.ak_hi, g.ak_lo) : 0;
-                cp_async8(as + r * LDA + kk, v ? (A + ro + ko) : A, v);
+            for (int j = 0; j < EB; ++j) cb[j] = colB[p / BK + (NP / BK) * j];
+        } else cb[0] = colB[p];
+        int stage = 0; unsigned par = 1;
+        for (int t = 0; t < total; ++t) {
+            const int ph = t >= nk ? 1 : 0;
+            const int kbase = (kt0 + (t - ph * nk)) * BK;
+            const double* A = Ap[ph];
+            const double* B = Bp[ph];
+            mbar_wait(&empty[stage], par);
+            double* as = As + stage * BM * LDA;
+            double* bs = Bs + stage * BK * LDB;
+            if (a_kfast) {
+                const int kk = p % BK, k = kbase + kk;
+                const bool kv = k < g.K;
+                const double* Ak = A + (kv ? (k1 ? (long long)k * g.ak_lo : idx2(k, g.Klo, g.ak_hi, g.ak_lo)) : 0);
+                double* d = as + (p / BK) * LDA + kk;
+#pragma unroll
+                for (int j = 0; j < EA; ++j) {
+                    const bool v = kv && ra[j] >= 0;
+                    cp_async8p(d + (NP / BK) * j * LDA, v ? Ak + ra[j] : A, v);
+                }
+            } else {
+                const bool rv = ra[0] >= 0;
+                const double* Ar = A + (rv ? ra[0] : 0);
+                double* d = as + p * LDA;
+                if (k1) {
+                    const double* s = Ar + (long long)kbase * g.ak_lo;
+#pragma unroll
+                    for (int j = 0; j < EA; ++j) {
+                        const bool v = rv && (kbase + j < g.K);
+                        cp_async8p(d + j, v ? s : A, v);
+                        s += g.ak_lo;
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < EA; ++j) {
+                        const bool v = rv && (kbase + j < g.K);
+                        cp_async8p(d + j, v ? Ar + idx2(kbase + j, g.Klo, g.ak_hi, g.ak_lo) : A, v);
+                    }
+                }
             }
+            if (b_nfast) {
+                const bool cv = cb[0] >= 0;
+                const double* Bc = B + (cv ? cb[0] : 0);
+                double* d = bs + p;
+                if (k1) {
+                    const double* s = Bc + (long long)kbase * g.bk_lo;
+#pragma unroll
+                    for (int j = 0; j < EB; ++j) {
+                        const bool v = cv && (kbase + j < g.K);
+                        cp_async8p(d + j * LDB, v ? s : B, v);
+                        s += g.bk_lo;
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < EB; ++j) {
+                        const bool v = cv && (kbase + j < g.K);
+                        cp_async8p(d + j * LDB, v ? Bc + idx2(kbase + j, g.Klo, g.bk_hi, g.bk_lo) : B, v);
+                    }
+                }
+            } else {
+                const int kk = p % BK, k = kbase + kk;
+                const bool kv = k < g.K;
+                const double* Bk = B + (kv ? (k1 ? (long long)k * g.bk_lo : idx2(k, g.Klo, g.bk_hi, g.bk_lo)) : 0);
+                double* d = bs + kk * LDB + p / BK;
+#pragma unroll
+                for (int j = 0; j < EB; ++j) {
+                    const bool v = kv && cb[j] >= 0;
+                    cp_async8p(d + (NP / BK) * j, v ? Bk + cb[j] : B, v);
+                }
+            }
+            cp_async_mbar_arrive(&full[stage]);
+            if (++stage == ST) { stage = 0; par ^= 1; }
         }
-        if (g.b_nfast) {
-            const int c = tid % BN, k0 = tid / BN;
-            const long long co = colB[c];
-#pragma unroll
-            for (int j = 0; j < EB; ++j) {
-                int kk = k0 + j * (NTH / BN);
-                int k = kbase + kk;
-                bool v = (k < g.K) && co >= 0;
-                long long ko = v ? idx2(k, g.Klo, g.bk_hi, g.bk_lo) : 0;
-                cp_async8(bs + kk * LDB + c, v ? (B + co + ko) : B, v);
-            }
-        } else {
-            const int kk = tid % BK, c0 = tid / BK;
-            const int k = kbase + kk;
-            const bool kv = k < g.K;
-            const long long ko = kv ? idx2(k, g.Klo, g.bk_hi, g.bk_lo) : 0;
-#pragma unroll
-            for (int j = 0; j < EB; ++j) {
-                int c = c0 + j * (NTH / BK);
-                long long co = colB[c];
-                bool v = kv && co >= 0;
-                cp_async8(bs + kk * LDB + c, v ? (B + co + ko) : B, v);
-            }
-        }
-    };
+        return;
+    }
 
+    // ---------------------------------------------------------------- consumers
     double acc[TM][TN][2];
 #pragma unroll
     for (int i = 0; i < TM; ++i)
@@ -168,42 +235,34 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32) tcgemm_kernel(cons
 
     const int wm0 = (warp / (BN / WN)) * WM, wn0 = (warp % (BN / WN)) * WN;
     const int lr = lane >> 2, lc = lane & 3;
-
-#pragma unroll
-    for (int s = 0; s < ST - 1; ++s) {
-        if (s < total) load_tile(s, s);
-        cp_async_commit();
-    }
+    const bool flip = nph == 2 && g.s0[db] != g.s1[db];
+    int stage = 0; unsigned par = 0;
     for (int t = 0; t < total; ++t) {
-        cp_async_wait<ST - 2>();
-        __syncthreads();
-        {
-            int tn = t + ST - 1;
-            if (tn < total) load_tile(tn, tn % ST);
-            cp_async_commit();
-        }
-        if (nph == 2 && t == nk && g.s0[db] != g.s1[db]) {
+        mbar_wait(&full[stage], par);
+        if (flip && t == nk) {
 #pragma unroll
             for (int i = 0; i < TM; ++i)
 #pragma unroll
                 for (int j = 0; j < TN; ++j) { acc[i][j][0] = -acc[i][j][0]; acc[i][j][1] = -acc[i][j][1]; }
         }
-        const double* as = As + (t % ST) * BM * LDA;
-        const double* bs = Bs + (t % ST) * BK * LDB;
+        const double* as = As + stage * BM * LDA + (wm0 + lr) * LDA + lc;
+        const double* bs = Bs + stage * BK * LDB + lc * LDB + wn0 + lr;
 #pragma unroll
         for (int ks = 0; ks < BK / 4; ++ks) {
             double a[TM], b[TN];
 #pragma unroll
-            for (int i = 0; i < TM; ++i) a[i] = as[(wm0 + 8 * i + lr) * LDA + ks * 4 + lc];
+            for (int i = 0; i < TM; ++i) a[i] = as[8 * i * LDA + ks * 4];
 #pragma unroll
-            for (int j = 0; j < TN; ++j) b[j] = bs[(ks * 4 + lc) * LDB + wn0 + 8 * j + lr];
+            for (int j = 0; j < TN; ++j) b[j] = bs[ks * 4 * LDB + 8 * j];
 #pragma unroll
             for (int i = 0; i < TM; ++i)
 #pragma unroll
                 for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[stage]);
+        if (++stage == ST) { stage = 0; par ^= 1; }
     }
-    cp_async_wait<0>();
 
     const double sgn = (nph == 2) ? (double)g.s1[db] : (double)g.s0[db];
     if (g.ksplit > 1) {
@@ -266,7 +325,7 @@ __global__ void tcgemm_splitk_reduce(const TcGemm g)
 
 template <int BM, int BN> constexpr size_t tcgemm_smem()
 {
-    return sizeof(double) * (3 * BM * (16 + 4) + 3 * 16 * (BN + 4)) + sizeof(long long) * (BM + BN);
+    return sizeof(double) * (4 * BM * (16 + 4) + 4 * 16 * (BN + 4)) + sizeof(long long) * (BM + BN) + 8 * sizeof(unsigned long long);
 }
 
 // Host launcher.  ws_cap = capacity (doubles) of g.ws; returns number of kernels launched (1 or 2).
@@ -303,9 +362,9 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     }
     dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, nbt * ks);
     if (big) {
-        tcgemm_kernel<128, 128, 64, 32><<<grid, 256, tcgemm_smem<128, 128>(), st>>>(g);
+        tcgemm_kernel<128, 128, 64, 32><<<grid, 384, tcgemm_smem<128, 128>(), st>>>(g);
     } else {
-        tcgemm_kernel<64, 64, 32, 32><<<grid, 128, tcgemm_smem<64, 64>(), st>>>(g);
+        tcgemm_kernel<64, 64, 32, 32><<<grid, 192, tcgemm_smem<64, 64>(), st>>>(g);
     }
     if (ks > 1) {
         long long tot = (long long)g.M * g.N * nbt;
