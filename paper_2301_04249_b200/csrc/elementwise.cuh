@@ -153,8 +153,8 @@ __global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const
     }
 }
 
-// Mq[Q][pl][(s,i,a)] += Lt[s][pl][Q][o+a][i]      (N^Q_ia = L~^Q_ai + M^Q_ia)
-__global__ void k_add_Lvo(Dims d, const double* __restrict__ Lt0, const double* __restrict__ Lt1, double* __restrict__ Mq)
+// Nq[Q][pl][(s,i,a)] = Mq + Lt[s][pl][Q][o+a][i]      (N^Q_ia = L~^Q_ai + M^Q_ia)
+__global__ void k_add_Lvo(Dims d, const double* __restrict__ Lt0, const double* __restrict__ Lt1, const double* __restrict__ Mq, double* __restrict__ Nq)
 {
     const long long tot = (long long)d.NQ * 2 * d.n1;
     const long long nn = (long long)d.n * d.n, plane = (long long)d.NQ * nn;
@@ -164,7 +164,7 @@ __global__ void k_add_Lvo(Dims d, const double* __restrict__ Lt0, const double* 
         int s = c >= d.n1a; int cc = s ? c - d.n1a : c;
         int i = cc / d.v[s], a = cc - i * d.v[s];
         const double* Lt = s ? Lt1 : Lt0;
-        Mq[x] += Lt[pl * plane + Q * nn + (long long)(d.o[s] + a) * d.n + i];
+        Nq[x] = Mq[x] + Lt[pl * plane + Q * nn + (long long)(d.o[s] + a) * d.n + i];
     }
 }
 

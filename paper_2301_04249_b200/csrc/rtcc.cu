@@ -21,9 +21,9 @@ struct rtcc_ctx {
     Dims d{};
     unsigned flags = 0;
     cudaStream_t st = nullptr;
-    cudaStream_t S[4]{};                 // S[0] = st (or the capture stream), S[1..3] = helper branches
-    cudaStream_t aux[3]{};
-    cudaEvent_t evs[8]{};
+    cudaStream_t S[8]{};                 // S[0] = st (or the capture stream), S[1..3] = helper branches
+    cudaStream_t aux[7]{};
+    cudaEvent_t evs[16]{};
     int si = 0;
     int num_sms = 148;
     int cuda_err = 0;
@@ -34,7 +34,7 @@ struct rtcc_ctx {
     double *L[2]{}, *Lt[2]{}, *fockd[2]{}, *Fb[2]{}, *Ft[2]{}, *Kx[2]{}, *KxBA = nullptr;
     double *t1r = nullptr, *Tsc = nullptr, *Wsc = nullptr, *Zsc = nullptr;
     double *TAB = nullptr, *WBB = nullptr, *WAA = nullptr, *ZAB = nullptr, *ZBA = nullptr;
-    double *Mq = nullptr, *gam = nullptr, *r1buf = nullptr;
+    double *Nq = nullptr, *Mq = nullptr, *gam = nullptr, *r1buf = nullptr;
     double *Xab = nullptr, *tauab = nullptr, *Yab = nullptr, *Wooab = nullptr;
     double *LtA[2]{}, *LtB[2]{}, *Xt_ab = nullptr, *Xt_ss[2]{};   // tile-major ladder operands
     int nt2_ab = 128, nt2_ss[2]{128, 128};
@@ -110,7 +110,7 @@ void ops_cc(TcGemm& g, const double* A, long long pA, const double* B, long long
 }
 void run(rtcc_ctx* c, TcGemm& g)
 {
-    const long long cap = c->ws_cap / 4;
+    const long long cap = c->ws_cap / 8;
     g.ws = c->ws + c->si * cap;
     int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops);
     c->launches += n;
@@ -137,7 +137,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     // captures into one CUDA graph with parallel branches).  Timing mode keeps everything on one stream.
     const bool par = !c->timing;
     c->S[0] = c->st;
-    for (int i = 0; i < 3; ++i) c->S[i + 1] = par ? c->aux[i] : c->st;
+    for (int i = 0; i < 7; ++i) c->S[i + 1] = par ? c->aux[i] : c->st;
 #define ST (c->S[c->si])
 #define BR(i) (c->si = (i))
 #define LINK(from, to, e) do { if (par) { CK(cudaEventRecord(c->evs[e], c->S[from])); CK(cudaStreamWaitEvent(c->S[to], c->evs[e], 0)); } } while (0)
@@ -210,6 +210,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         run(c, g);
     }
 
+    if (par) CK(cudaEventRecord(c->evs[6], c->S[0]));     // evs[6]: gamma, M ready
+
     // ---- 5. E (needs the bare M^Q)
     {
         EnergyArgs ea;
@@ -225,6 +227,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
         double* F = c->Ft[s];
+        if (s == 1) { if (par) CK(cudaEventRecord(c->evs[2], c->S[0])); BR(4); WAITEV(4, 6); }   // evs[2]: spin-0 F ready
         CK(cudaMemcpyAsync(F, c->Fb[s], nn * 8, cudaMemcpyDeviceToDevice, ST));
         CK(cudaMemsetAsync(F + nn, 0, nn * 8, ST));
         {
@@ -285,7 +288,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         }
     }
 
-    if (par) CK(cudaEventRecord(c->evs[2], c->S[0]));     // evs[2]: F intermediates ready
+    if (par) CK(cudaEventRecord(c->evs[7], c->S[4]));     // evs[7]: spin-1 F ready
+    WAITEV(4, 2);                                         // singles stay on branch 4
 
     // ---- 7. singles:  r1 = sum_me t_im^ae f~_me - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af   (+ f~_ai at assembly)
     for (int s = 0; s < 2; ++s) {
@@ -324,13 +328,14 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 8. driver + Coulomb ring channel:  Zsc = 1/2 N^T N,  N^Q_ia = L~^Q_ai + M^Q_ia
-    EW(c, k_add_Lvo, (long long)NQ * 2 * n1, d, c->Lt[0], c->Lt[1], c->Mq);
+    BR(0);
+    EW(c, k_add_Lvo, (long long)NQ * 2 * n1, d, c->Lt[0], c->Lt[1], c->Mq, c->Nq);
     {
         TcGemm g = G0(n1, n1, NQ);
         setA(g, 0, 1, 0, 0, ld1, 0, 0);
         setB(g, 0, ld1, 0, 1, 0, 1);
         setC(g, 0, ld1, 0, 1);
-        ops_cc(g, c->Mq, n1, c->Mq, n1, c->Zsc, n1);
+        ops_cc(g, c->Nq, n1, c->Nq, n1, c->Zsc, n1);
         g.alpha = 0.5;
         run(c, g);
     }
@@ -360,7 +365,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             g.beta = 1.0;
             run(c, g);
         }
-        if (s == 0 || d.n1a == 0) WAITEV(1, 2);
+        if (s == 0 || d.n1a == 0) { WAITEV(1, 2); WAITEV(1, 7); }
         EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1);
     }
     LINK(1, 0, 3);
@@ -400,6 +405,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             run(c, g);
         }
         WAITEV(2, 2);
+        WAITEV(2, 7);
         EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL);
         {
             TcGemm g = G0(nA, nB, nB);
@@ -448,13 +454,15 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], ST));
-    WAITEV(3, 1);
+    if (par) CK(cudaEventRecord(c->evs[9], c->S[3]));     // evs[9]: ladder output ready
 
     if (d.oo > 0) {
         const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], oo = d.oo;
         const long long lY = 2LL * oo;
         double* Yvv = c->Yab + ((long long)oa * n + ob) * lY;
-        {   // <mN||iJ>~ = sum_Q L~_mi L~_NJ
+        BR(7);
+        WAITEV(7, 1);
+        {   // <mN||iJ>~ = sum_Q L~_mi L~_NJ   (independent of the ladder: own branch)
             TcGemm g = G0(oa * oa, ob * ob, NQ);
             setA(g, n, 1, oa, 0, nn, 0, 0);
             setB(g, 0, nn, n, 1, ob, 1);
@@ -462,6 +470,9 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             ops_cc(g, c->Lt[0], plane, c->Lt[1], plane, c->Wooab, oo);
             run(c, g);
         }
+        if (par) CK(cudaEventRecord(c->evs[8], c->S[7]));
+        BR(3);
+        WAITEV(3, 8);
         {   // + t_mN^aB <mN||iJ>~
             TcGemm g = G0(va * vb, oo, oo);
             setA(g, vb * lY, lY, vb, 0, 1, 0, 1);
@@ -506,6 +517,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         if (po == 0) continue;
         const long long lP = 2LL * po, o2 = (long long)o * o;
         double* Yvv = c->Yss[s] + ((long long)o * n + o) * lP;
+        BR(7);
+        WAITEV(7, 1);
         {
             TcGemm g = G0(o * o, o * o, NQ);
             setA(g, n, 1, o, 0, nn, 0, 0);
@@ -514,6 +527,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             ops_cc(g, c->Lt[s], plane, c->Lt[s], plane, c->W4[s], o2);
             run(c, g);
         }
+        if (par) CK(cudaEventRecord(c->evs[13 + s], c->S[7]));
+        BR(5 + s);
+        WAITEV(5 + s, 9);
+        WAITEV(5 + s, 13 + s);
         EW(c, k_ss_prep, (long long)po * po, o, po, n, c->opairs[s], c->W4[s], c->Yss[s], c->Wp[s], c->Yoop[s]);
         {
             TcGemm g = G0(v * v, po, po);
@@ -545,6 +562,9 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
 
     LINK(2, 0, 4);
     LINK(3, 0, 5);
+    LINK(4, 0, 10);
+    if (d.po[0] > 0) LINK(5, 0, 11);
+    if (d.po[1] > 0) LINK(6, 0, 12);
     BR(0);
 
     // ---- 12. antisymmetrise and write the packed residual
@@ -636,8 +656,8 @@ void rtcc_destroy(rtcc_ctx* c)
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->ev[0]) cudaEventDestroy(c->ev[0]);
     if (c->ev[1]) cudaEventDestroy(c->ev[1]);
-    for (int i = 0; i < 3; ++i) if (c->aux[i]) cudaStreamDestroy(c->aux[i]);
-    for (int i = 0; i < 8; ++i) if (c->evs[i]) cudaEventDestroy(c->evs[i]);
+    for (int i = 0; i < 7; ++i) if (c->aux[i]) cudaStreamDestroy(c->aux[i]);
+    for (int i = 0; i < 16; ++i) if (c->evs[i]) cudaEventDestroy(c->evs[i]);
     for (void* p : c->allocs) cudaFree(p);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -681,9 +701,10 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(ladder_init());
         CKC(cudaEventCreate(&c->ev[0]));
         CKC(cudaEventCreate(&c->ev[1]));
-        for (int i = 0; i < 3; ++i) CKC(cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking));
-        for (int i = 0; i < 8; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
-        c->S[0] = c->S[1] = c->S[2] = c->S[3] = c->st; c->si = 0;
+        for (int i = 0; i < 7; ++i) CKC(cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 16; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
+        for (int i = 0; i < 8; ++i) c->S[i] = c->st;
+        c->si = 0;
         CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
 
         for (int s = 0; s < 2; ++s) {
@@ -728,6 +749,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
         DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
         DA(c->Mq, 2LL * NQ * n1, "Mq");
+        DA(c->Nq, 2LL * NQ * n1, "Nq");
         DA(c->gam, 2LL * NQ, "gam");
         DA(c->r1buf, 2LL * n1, "r1buf");
         DA(c->Xab, (long long)va * vb * 2 * d.oo, "Xab");
@@ -742,7 +764,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
         DA(c->Yab, nn * 2 * d.oo, "Yab");
         DA(c->Wooab, (long long)d.oo * 2 * d.oo, nullptr);
-        c->ws_cap = 16LL << 20;
+        c->ws_cap = 32LL << 20;
         DA(c->ws, c->ws_cap, nullptr);
         DA(c->partial, 2 * RED_BLOCKS, nullptr);
         DA(c->bmax, RED_BLOCKS, nullptr);

@@ -35,6 +35,7 @@ struct TcGemm {
     long long sbA, sbB, sbC;
     double alpha, beta;
     int a_kfast, b_nfast;                    // which index of A / B is contiguous in memory
+    int a_klin, b_klin;                      // k index of A / B is effectively single-level (set by the launcher)
     int ksplit;                              // deterministic split-K (partials in ws, reduced by a 2nd kernel)
     double* ws;
 };
@@ -138,7 +139,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
         const int p = tid - NCW * 32;
         const double* Ap[2] = {g.A[db][0] + sb * g.sbA, g.A[db][1] + sb * g.sbA};
         const double* Bp[2] = {g.B[db][0] + sb * g.sbB, g.B[db][1] + sb * g.sbB};
-        const bool k1 = g.Klo >= 0x40000000;            // single-level k
+        const bool k1a = g.a_klin, k1b = g.b_klin;      // single-level k per operand
         const int a_kfast = g.a_kfast, b_nfast = g.b_nfast;
         // kfast: this thread owns k-column (p % 16) of rows p/16 + (NP/16) j;  otherwise row p, all 16 k
         long long ra[EA];                               // row offsets (kfast) -- or ra[0] only
@@ -163,7 +164,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
             if (a_kfast) {
                 const int kk = p % BK, k = kbase + kk;
                 const bool kv = k < g.K;
-                const double* Ak = A + (kv ? (k1 ? (long long)k * g.ak_lo : idx2(k, g.Klo, g.ak_hi, g.ak_lo)) : 0);
+                const double* Ak = A + (kv ? (k1a ? (long long)k * g.ak_lo : idx2(k, g.Klo, g.ak_hi, g.ak_lo)) : 0);
                 double* d = as + (p / BK) * LDA + kk;
 #pragma unroll
                 for (int j = 0; j < EA; ++j) {
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
                 const bool rv = ra[0] >= 0;
                 const double* Ar = A + (rv ? ra[0] : 0);
                 double* d = as + p * LDA;
-                if (k1) {
+                if (k1a) {
                     const double* s = Ar + (long long)kbase * g.ak_lo;
 #pragma unroll
                     for (int j = 0; j < EA; ++j) {
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
                 const bool cv = cb[0] >= 0;
                 const double* Bc = B + (cv ? cb[0] : 0);
                 double* d = bs + p;
-                if (k1) {
+                if (k1b) {
                     const double* s = Bc + (long long)kbase * g.bk_lo;
 #pragma unroll
                     for (int j = 0; j < EB; ++j) {
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
             } else {
                 const int kk = p % BK, k = kbase + kk;
                 const bool kv = k < g.K;
-                const double* Bk = B + (kv ? (k1 ? (long long)k * g.bk_lo : idx2(k, g.Klo, g.bk_hi, g.bk_lo)) : 0);
+                const double* Bk = B + (kv ? (k1b ? (long long)k * g.bk_lo : idx2(k, g.Klo, g.bk_hi, g.bk_lo)) : 0);
                 double* d = bs + kk * LDB + p / BK;
 #pragma unroll
                 for (int j = 0; j < EB; ++j) {
@@ -334,6 +335,8 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     if (g.M <= 0 || g.N <= 0 || g.nb <= 0 || g.nsb <= 0) return 0;
     if (g.Mlo <= 0 || g.Mlo >= g.M) g.Mlo = 0x40000000;
     if (g.Nlo <= 0 || g.Nlo >= g.N) g.Nlo = 0x40000000;
+    g.a_klin = (g.Klo <= 0 || g.Klo >= g.K) || g.ak_hi == (long long)g.Klo * g.ak_lo;
+    g.b_klin = (g.Klo <= 0 || g.Klo >= g.K) || g.bk_hi == (long long)g.Klo * g.bk_lo;
     if (g.Klo <= 0 || g.Klo >= g.K) g.Klo = 0x40000000;
     const int nbt = g.nb * g.nsb;
     const long long t128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * nbt;
