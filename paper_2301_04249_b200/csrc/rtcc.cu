@@ -450,7 +450,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     BR(3);
     WAITEV(3, 0);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
-    c->launches += ladder_launch(c->lb, ST, c->num_sms);
+    if (!getenv("RTCC_SKIP_LADDER")) c->launches += ladder_launch(c->lb, ST, c->num_sms);   // (debug knob: timing of the other branches)
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], ST));
@@ -701,7 +701,13 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(ladder_init());
         CKC(cudaEventCreate(&c->ev[0]));
         CKC(cudaEventCreate(&c->ev[1]));
-        for (int i = 0; i < 7; ++i) CKC(cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking));
+        {   // helper branches: everything latency-bound outranks the SM-filling ladder branch (aux[2] = S[3])
+            int lo = 0, hi = 0;
+            CKC(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            const bool prio = !getenv("RTCC_NO_PRIO");
+            for (int i = 0; i < 7; ++i)
+                CKC(cudaStreamCreateWithPriority(&c->aux[i], cudaStreamNonBlocking, (prio && i != 2) ? hi : lo));
+        }
         for (int i = 0; i < 16; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
         for (int i = 0; i < 8; ++i) c->S[i] = c->st;
         c->si = 0;
@@ -828,7 +834,11 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
-            ladder_plan(B, c->num_sms, 8);
+            // SMs given to the (persistent) ladder kernel; the rest stay free for the concurrent latency-bound branches
+            int lsm = c->num_sms;
+            if (const char* e = getenv("RTCC_LADDER_SMS")) lsm = atoi(e);
+            if (lsm < 1 || lsm > c->num_sms) lsm = c->num_sms;
+            ladder_plan(B, lsm, 8);
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;

@@ -71,9 +71,12 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* b)
 { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity)
 {
-    asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
-        ::"r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+    const unsigned addr = (unsigned)__cvta_generic_to_shared(b);
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
 }
 // the barrier receives one arrival when all cp.async issued so far by this thread have landed
 __device__ __forceinline__ void cp_async_mbar_arrive(unsigned long long* b)
