@@ -367,3 +367,26 @@ def test_separability():
         C.append(pr.C)
     assert abs(C[2] - (C[0] + C[1])) < 1e-13
     assert abs(C[0]) > 1e-6 and abs(C[1]) > 1e-6
+
+
+# ------------------------------------------------------------------ tier B: sampled-element oracle vs tier A
+def test_sampled_oracle_matches_full_oracle():
+    """The on-demand-integral evaluation of single residual elements (oracle/sampled.py) must reproduce the full
+    spin-orbital oracle (pinned above by determinant-space brute force) on complex amplitudes, general Fock."""
+    from oracle.sampled import SampledOracle
+    for (oa, ob, va, vb, K, seed) in [(2, 3, 4, 3, 5, 21), (3, 1, 2, 4, 4, 22), (2, 2, 3, 3, 6, 23)]:
+        L, fock = rand_problem(oa, ob, va, vb, K, seed)
+        prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+        t1p, t2p = rand_amps(prob.d, seed + 100)
+        r1p, r2p, E = prob.residual(t1p, t2p)
+        so = SampledOracle(oa, ob, va, vb, K, L, fock, t1p, t2p)
+        assert abs(so.energy() - E) < 1e-13
+        for k in range(prob.d.n_t2):                  # every packed element, through the packed -> spin-orbital map
+            i, j, a, b = so.so_of_packed_t2(k)
+            assert abs(so.r2(i, j, a, b) - r2p[k]) < 1e-13, (k, i, j, a, b)
+        for k in range(prob.d.n_t1):
+            i, a = so.so_of_packed_t1(k)
+            assert abs(so.r1(i, a) - r1p[k]) < 1e-13
+        # antisymmetry of the sampled values themselves
+        i, j, a, b = so.so_of_packed_t2(0)
+        assert abs(so.r2(j, i, a, b) + so.r2(i, j, a, b)) < 1e-13

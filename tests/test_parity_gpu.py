@@ -192,3 +192,39 @@ def test_contraction_primitive_against_matmul(rtcc):
         assert np.abs(rtcc.debug_gemm(A, B, C, 0.7, -0.3) - ref).max() <= 1e-12 * np.abs(ref).max()
         ref = 0.7 * A.real @ B.real - 0.3 * C.real
         assert np.abs(rtcc.debug_gemm(A.real, B.real, C.real, 0.7, -0.3) - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("amp_std", [1e-3, 3e-2])
+def test_residual_small_config_full_size_sampled(rtcc, amp_std):
+    """BASELINE.json config 2 (Small: o=8, v=60, n_chol=340) at FULL size, literal generator, in the launch configuration
+    bench.py times (CUDA-graph replay, device pointers): seeded sample of residual elements from all three spin blocks, all
+    checked against the sampled-element oracle (oracle/sampled.py, itself pinned to the full oracle), plus E."""
+    import torch
+    from oracle.sampled import SampledOracle
+    cfg = inputs.CONFIGS["small"]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg)
+    t1, t2 = inputs.random_amplitudes(cfg, std=amp_std)
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda())
+    r1d, r2d = ctx.residual(torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda())
+    r1, r2 = r1d.cpu().numpy(), r2d.cpu().numpy()
+    E = ctx.residual_energy()
+    ctx.close()
+    assert np.isfinite(r1).all() and np.isfinite(r2).all()
+    scale = max(np.abs(r1).max(), np.abs(r2).max())
+    so = SampledOracle(oa, ob, va, vb, K, L, fock, t1, t2)
+    d = so.d
+    naa = orc.npair(oa) * orc.npair(va)
+    nbb = orc.npair(ob) * orc.npair(vb)
+    rng = np.random.default_rng(4249)
+    picks = [0, naa - 1, naa, naa + nbb - 1, naa + nbb, d.n_t2 - 1]            # block boundaries
+    picks += list(rng.integers(0, naa, 40)) + list(naa + rng.integers(0, nbb, 40)) + list(naa + nbb + rng.integers(0, d.n_t2 - naa - nbb, 80))
+    worst = 0.0
+    for k in picks:
+        i, j, a, b = so.so_of_packed_t2(int(k))
+        worst = max(worst, abs(so.r2(i, j, a, b) - r2[int(k)]))
+    for k in list(rng.integers(0, d.n_t1, 30)) + [0, d.n_t1 - 1]:
+        i, a = so.so_of_packed_t1(int(k))
+        worst = max(worst, abs(so.r1(i, a) - r1[int(k)]))
+    assert worst <= RTOL * scale, (worst, scale)
+    Eo = so.energy()
+    assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
