@@ -43,7 +43,6 @@ struct LadderCase {
 };
 struct LadderBatch {
     LadderCase c[3];
-    int grid;                             // persistent CTAs (<= nitems)
     int ncase, NQ, nitems;                // NQ: padded to a multiple of 16
 };
 
@@ -65,27 +64,36 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_inval(unsigned long long* b)
-{ asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"((unsigned)__cvta_generic_to_shared(b)) : "memory"); }
 __device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
-// Producer side of one work item (one elected lane): the ring position (stage, par) carries over between items.
 template <int NT2>
-__device__ __forceinline__ void ladder_produce(const LadderCase& gc, const int NQ, const int p0, const int q0, const int x0,
-                                               const int ch_begin, const int ch_end, double* smem, int& stage, unsigned& par)
+__device__ __forceinline__ void ladder_body(const LadderCase& gc, const int NQ, const int p0, const int q0, const int x0,
+                                            const int ch_begin, const int ch_end, double* __restrict__ Yout, double* smem)
 {
     constexpr int LDX2 = NT2 + 4;
+    constexpr int WGN = NT2 / 32;               // GEMM-2 warp grid: (8/WGN) x WGN, warp tile WM2 x 32
+    constexpr int WGM = 8 / WGN;
+    constexpr int WM2 = LD_R / WGM;             // 32 (NT2=128) or 16 (NT2=64)
+    constexpr int TM2 = WM2 / 8;
     double* stg = smem;
     double* Ws = smem + LD_ST * LD_STAGE;
     unsigned long long* full = reinterpret_cast<unsigned long long*>(Ws + LD_R * LD_LDW);
     unsigned long long* empty = full + LD_ST;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nFt = (gc.vB + LD_PF - 1) / LD_PF;
     const int T1 = NQ / LD_BK;
     constexpr int T2 = LD_K2 / LD_BK;
     const int tpc = T1 + T2;
     const int total = (ch_end - ch_begin) * tpc;
-    (void)Ws; (void)warp;
+
+    if (tid == 0) {
+        for (int s = 0; s < LD_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == 8) {
         // ---------------- producer: one elected lane, one or two bulk copies per tile
         if (lane == 0) {
             const int nEt = (gc.vA + LD_PE - 1) / LD_PE;
@@ -97,6 +105,7 @@ __device__ __forceinline__ void ladder_produce(const LadderCase& gc, const int N
             const double* curA = LAp + (long long)et * T1 * BLKA;
             const double* curB = LBp + (long long)ft * T1 * BLKB;
             const double* curX = gc.X + (((long long)(et * nFt + ft) * ncol + ct) * T2) * BLKX;
+            int stage = 0; unsigned par = 1;       // first pass over the ring: slots are free
             for (int it = 0; it < total; ++it) {
                 mbar_wait(&empty[stage], par);
                 double* sb = stg + stage * LD_STAGE;
@@ -120,30 +129,9 @@ __device__ __forceinline__ void ladder_produce(const LadderCase& gc, const int N
                 if (++stage == LD_ST) { stage = 0; par ^= 1; }
             }
         }
-}
+        return;
+    }
 
-// Consumer side of one work item (8 warps).
-template <int NT2>
-__device__ __forceinline__ void ladder_consume(const LadderCase& gc, const int NQ, const int p0, const int q0, const int x0,
-                                               const int ch_begin, const int ch_end, double* __restrict__ Yout, double* smem,
-                                               int& stage, unsigned& par)
-{
-    constexpr int LDX2 = NT2 + 4;
-    double* stg = smem;
-    double* Ws = smem + LD_ST * LD_STAGE;
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(Ws + LD_R * LD_LDW);
-    unsigned long long* empty = full + LD_ST;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nFt = (gc.vB + LD_PF - 1) / LD_PF;
-    const int T1 = NQ / LD_BK;
-    constexpr int T2 = LD_K2 / LD_BK;
-    const int tpc = T1 + T2;
-    const int total = (ch_end - ch_begin) * tpc;
-    constexpr int WGN = NT2 / 32;               // GEMM-2 warp grid: (8/WGN) x WGN, warp tile WM2 x 32
-    constexpr int WGM = 8 / WGN;
-    constexpr int WM2 = LD_R / WGM;             // 32 (NT2=128) or 16 (NT2=64)
-    constexpr int TM2 = WM2 / 8;
-    (void)empty;
     // ---------------- consumer warps
     const int lr = lane >> 2, lc = lane & 3;
     double acc2[TM2][4][2];
@@ -157,7 +145,7 @@ __device__ __forceinline__ void ladder_consume(const LadderCase& gc, const int N
     const int w1m = (warp >> 1) * 32, w1n = (warp & 1) * 32;
     const int w2m = (warp / WGN) * WM2, w2n = (warp % WGN) * 32;
 
-    int r = 0;
+    int r = 0, stage = 0; unsigned par = 0;
     for (int it = 0; it < total; ++it) {
         mbar_wait(&full[stage], par);
         const double* sb = stg + stage * LD_STAGE;
@@ -239,59 +227,24 @@ __device__ __forceinline__ void ladder_consume(const LadderCase& gc, const int N
     }
 }
 
-struct LadderItem { int ci, p0, q0, col, ch0, ch1; double* Yout; };
-__device__ __forceinline__ LadderItem ladder_decode(const LadderBatch& b, int item)
-{
-    LadderItem t;
-    t.ci = 0;
-    if (b.ncase > 1 && item >= b.c[1].item0) t.ci = 1;
-    if (b.ncase > 2 && item >= b.c[2].item0) t.ci = 2;
-    const LadderCase& g = b.c[t.ci];
-    item -= g.item0;
-    const int split = item % g.nsplit; item /= g.nsplit;
-    t.col = item % g.ncol;
-    const int2 tl = g.tiles[item / g.ncol];
-    t.p0 = tl.x; t.q0 = tl.y;
-    const int nchunk = ((g.vA + LD_PE - 1) / LD_PE) * ((g.vB + LD_PF - 1) / LD_PF);
-    t.ch0 = (int)((long long)split * nchunk / g.nsplit);
-    t.ch1 = (int)((long long)(split + 1) * nchunk / g.nsplit);
-    t.Yout = g.nsplit > 1 ? g.Ypart + (long long)split * g.nA * g.nB * g.ldY : g.Y;
-    return t;
-}
-
-// Persistent: the grid may be smaller than the item list (SMs are left free for the latency-bound branches of the
-// residual graph that run concurrently); items are equal-sized, so a static round-robin is balanced.  Producer and
-// consumers walk the same item sequence; the mbarrier ring simply continues across items.
-__global__ void __launch_bounds__(LD_NTH, 1) ladder_kernel(const LadderBatch b)
+__global__ void __launch_bounds__(LD_NTH) ladder_kernel(const LadderBatch b)
 {
     extern __shared__ __align__(128) double smem[];
-    {
-        double* Ws = smem + LD_ST * LD_STAGE;
-        unsigned long long* full = reinterpret_cast<unsigned long long*>(Ws + LD_R * LD_LDW);
-        unsigned long long* empty = full + LD_ST;
-        if (threadIdx.x == 0) {
-            for (int s = 0; s < LD_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncthreads();
-    }
-    if ((threadIdx.x >> 5) == 8) {
-        int stage = 0; unsigned par = 1;           // first pass over the ring: slots are free
-        for (int it = blockIdx.x; it < b.nitems; it += gridDim.x) {
-            const LadderItem t = ladder_decode(b, it);
-            const LadderCase& g = b.c[t.ci];
-            if (g.nt2 == 64) ladder_produce<64>(g, b.NQ, t.p0, t.q0, t.col * 64, t.ch0, t.ch1, smem, stage, par);
-            else ladder_produce<128>(g, b.NQ, t.p0, t.q0, t.col * 128, t.ch0, t.ch1, smem, stage, par);
-        }
-    } else {
-        int stage = 0; unsigned par = 0;
-        for (int it = blockIdx.x; it < b.nitems; it += gridDim.x) {
-            const LadderItem t = ladder_decode(b, it);
-            const LadderCase& g = b.c[t.ci];
-            if (g.nt2 == 64) ladder_consume<64>(g, b.NQ, t.p0, t.q0, t.col * 64, t.ch0, t.ch1, t.Yout, smem, stage, par);
-            else ladder_consume<128>(g, b.NQ, t.p0, t.q0, t.col * 128, t.ch0, t.ch1, t.Yout, smem, stage, par);
-        }
-    }
+    int item = blockIdx.x, ci = 0;
+    if (b.ncase > 1 && item >= b.c[1].item0) ci = 1;
+    if (b.ncase > 2 && item >= b.c[2].item0) ci = 2;
+    const LadderCase& g = b.c[ci];
+    item -= g.item0;
+    const int split = item % g.nsplit; item /= g.nsplit;
+    const int col = item % g.ncol;
+    const int tile = item / g.ncol;
+    const int2 tl = g.tiles[tile];
+    const int nEt = (g.vA + LD_PE - 1) / LD_PE, nFt = (g.vB + LD_PF - 1) / LD_PF;
+    const int nchunk = nEt * nFt;
+    const int ch0 = (int)((long long)split * nchunk / g.nsplit), ch1 = (int)((long long)(split + 1) * nchunk / g.nsplit);
+    double* Yout = g.nsplit > 1 ? g.Ypart + (long long)split * g.nA * g.nB * g.ldY : g.Y;
+    if (g.nt2 == 64) ladder_body<64>(g, b.NQ, tl.x, tl.y, col * 64, ch0, ch1, Yout, smem);
+    else ladder_body<128>(g, b.NQ, tl.x, tl.y, col * 128, ch0, ch1, Yout, smem);
 }
 
 // Y = sum over slices of Ypart (fixed order)
@@ -337,7 +290,6 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
         item += g.ntiles * g.ncol * g.nsplit;
     }
     b.nitems = item;
-    b.grid = item < num_sms ? item : num_sms;
 }
 
 // executed tensor-pipe flops of one launch
@@ -355,7 +307,7 @@ inline double ladder_flops(const LadderBatch& b)
 inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
 {
     if (b.nitems <= 0) return 0;
-    ladder_kernel<<<b.grid, LD_NTH, ladder_smem(), st>>>(b);
+    ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(b);
     bool red = false;
     for (int i = 0; i < b.ncase; ++i) red |= b.c[i].nsplit > 1;
     if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); return 2; }

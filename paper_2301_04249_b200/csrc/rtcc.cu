@@ -25,6 +25,7 @@ struct rtcc_ctx {
     cudaStream_t aux[7]{};
     cudaEvent_t evs[16]{};
     int si = 0;
+    int sec = 0; unsigned skipmask = 0;   // debug: RTCC_SKIP_MASK skips the GEMMs of pipeline sections (timing experiments only)
     int num_sms = 148;
     int cuda_err = 0;
     std::vector<void*> allocs;
@@ -110,6 +111,7 @@ void ops_cc(TcGemm& g, const double* A, long long pA, const double* B, long long
 }
 void run(rtcc_ctx* c, TcGemm& g)
 {
+    if ((c->skipmask >> c->sec) & 1u) return;
     const long long cap = c->ws_cap / 8;
     g.ws = c->ws + c->si * cap;
     int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops);
@@ -145,6 +147,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     BR(0);
 
     // ---- 1. unpack the packed spin blocks into the contraction layouts
+    c->sec = 1;
     EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
     EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc);
     EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB);
@@ -156,6 +159,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
 
     // ---- 2. T1-dressed Cholesky vectors  L~^Q = (1-T) L^Q (1+T)
+    c->sec = 2;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -185,6 +189,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     if (par) CK(cudaEventRecord(c->evs[1], c->S[0]));     // evs[1]: dressed vectors ready
 
     // ---- 3. gamma^Q = sum_ie L^Q_ie t_i^e (both spins)
+    c->sec = 3;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -198,6 +203,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 4. M^Q_ia = sum_me L^Q_me t_im^ae over the spin-conserving pair space
+    c->sec = 4;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -213,6 +219,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     if (par) CK(cudaEventRecord(c->evs[6], c->S[0]));     // evs[6]: gamma, M ready
 
     // ---- 5. E (needs the bare M^Q)
+    c->sec = 5;
     {
         EnergyArgs ea;
         for (int s = 0; s < 2; ++s) { ea.L[s] = c->L[s]; ea.Lt[s] = c->Lt[s]; ea.fock[s] = c->fockd[s]; }
@@ -223,6 +230,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 6. dressed Fock  f~ = X (f + K_bare + sum_Q gamma^Q L^Q) Y - sum_Q,i L~^Q_pi L~^Q_iq
+    c->sec = 6;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -292,6 +300,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     WAITEV(4, 2);                                         // singles stay on branch 4
 
     // ---- 7. singles:  r1 = sum_me t_im^ae f~_me - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af   (+ f~_ai at assembly)
+    c->sec = 7;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -328,6 +337,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 8. driver + Coulomb ring channel:  Zsc = 1/2 N^T N,  N^Q_ia = L~^Q_ai + M^Q_ia
+    c->sec = 8;
     BR(0);
     EW(c, k_add_Lvo, (long long)NQ * 2 * n1, d, c->Lt[0], c->Lt[1], c->Mq, c->Nq);
     {
@@ -341,6 +351,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 9. exchange ring channel + F terms, spin-conserving sector:  Zsc -= T (Xd + 1/2 Kx T + Fd)
+    c->sec = 9;
     BR(1);
     WAITEV(1, 1);
     for (int s = 0; s < 2; ++s) {
@@ -381,6 +392,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 10. spin-flip sector
+    c->sec = 10;
     BR(2);
     WAITEV(2, 1);
     if (d.nA > 0 && d.nB > 0) {
@@ -447,6 +459,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     }
 
     // ---- 11. ladders (pp with all-orbital rows; hh and the T1 corrections from the occupied rows)
+    c->sec = 11;
     BR(3);
     WAITEV(3, 0);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
@@ -568,6 +581,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     BR(0);
 
     // ---- 12. antisymmetrise and write the packed residual
+    c->sec = 12;
     {
         AsmArgs A;
         A.Zsc = c->Zsc; A.ZAB = c->ZAB; A.ZBA = c->ZBA; A.Yab = c->Yab; A.r1buf = c->r1buf;
@@ -711,6 +725,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         for (int i = 0; i < 16; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
         for (int i = 0; i < 8; ++i) c->S[i] = c->st;
         c->si = 0;
+        if (const char* e = getenv("RTCC_SKIP_MASK")) c->skipmask = (unsigned)strtoul(e, nullptr, 0);
         CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
 
         for (int s = 0; s < 2; ++s) {
@@ -834,11 +849,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
-            // SMs given to the (persistent) ladder kernel; the rest stay free for the concurrent latency-bound branches
-            int lsm = c->num_sms;
-            if (const char* e = getenv("RTCC_LADDER_SMS")) lsm = atoi(e);
-            if (lsm < 1 || lsm > c->num_sms) lsm = c->num_sms;
-            ladder_plan(B, lsm, 8);
+            ladder_plan(B, c->num_sms, 8);
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;
