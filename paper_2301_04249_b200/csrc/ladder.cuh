@@ -39,6 +39,8 @@ struct LadderCase {
     int nsplit;                           // slices of the (e,f) chunk list
     int nt2;                              // column tile width: 64 or 128
     int ncol;                             // column tiles
+    int cl;                               // CTAs per cluster sharing one W chunk (1: plain kernel); ncol > 1 only
+    int ngrp;                             // column-tile groups of cl tiles each
     int item0;                            // first work item of this case
 };
 struct LadderBatch {
@@ -247,6 +249,230 @@ __global__ void __launch_bounds__(LD_NTH) ladder_kernel(const LadderBatch b)
     else ladder_body<128>(g, b.NQ, tl.x, tl.y, col * 128, ch0, ch1, Yout, smem);
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Wide amplitudes (more than one column tile): a thread-block CLUSTER of cl CTAs owns one (p,q) row tile.  CTA r
+// keeps the accumulators of column tile r.  Each W chunk is built ONCE per cluster: the n_chol reduction of GEMM-1 is
+// split across the CTAs, the partial tiles are summed through distributed shared memory in a fixed order
+// (reduce-scatter + all-gather, deterministic) and every CTA then applies the complete chunk to its own columns.
+constexpr int LC_ST = 3;
+constexpr size_t ladder_cluster_smem()
+{ return sizeof(double) * (LC_ST * (size_t)LD_STAGE + 2 * (size_t)LD_R * LD_LDW) + (2 * LC_ST + 2) * sizeof(unsigned long long); }
+
+__device__ __forceinline__ unsigned cluster_rank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ unsigned map_shared(const void* p, unsigned rank)
+{
+    unsigned a = (unsigned)__cvta_generic_to_shared(p), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ double2 ld_cluster2(unsigned addr)
+{ double2 v; asm volatile("ld.shared::cluster.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory"); return v; }
+__device__ __forceinline__ void st_cluster2(unsigned addr, double2 v)
+{ asm volatile("st.shared::cluster.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory"); }
+__device__ __forceinline__ void mbar_arrive_cluster(unsigned remote_addr)
+{ asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote_addr) : "memory"); }
+__device__ __forceinline__ void mbar_wait_cluster(unsigned long long* b, unsigned parity)
+{
+    const unsigned addr = (unsigned)__cvta_generic_to_shared(b);
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+__global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderCase g, const int NQ)
+{
+    constexpr int NT2 = 128, LDX2 = NT2 + 4, T2 = LD_K2 / LD_BK;
+    extern __shared__ __align__(128) double smem[];
+    double* stg = smem;
+    double* Ws = smem + LC_ST * LD_STAGE;
+    double* Ps = Ws + LD_R * LD_LDW;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(Ps + LD_R * LD_LDW);
+    unsigned long long* empty = full + LC_ST;
+    unsigned long long* cbar = empty + LC_ST;          // [0]: partial tiles written, [1]: reduced chunk distributed
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int cl = g.cl;
+    const int rank = (int)cluster_rank();
+    int item = blockIdx.x / cl;
+    const int split = item % g.nsplit; item /= g.nsplit;
+    const int grp = item % g.ngrp;
+    const int2 tl = g.tiles[item / g.ngrp];
+    const int p0 = tl.x, q0 = tl.y;
+    const int col = grp * cl + rank;
+    const bool has_col = col < g.ncol;
+    const int x0 = col * NT2;
+    const int nEt = (g.vA + LD_PE - 1) / LD_PE, nFt = (g.vB + LD_PF - 1) / LD_PF;
+    const int nchunk = nEt * nFt;
+    const int ch0 = (int)((long long)split * nchunk / g.nsplit), ch1 = (int)((long long)(split + 1) * nchunk / g.nsplit);
+    const int T1 = NQ / LD_BK;
+    const int kt0 = (int)((long long)rank * T1 / cl), kt1 = (int)((long long)(rank + 1) * T1 / cl);   // my share of the n_chol reduction
+    const int T1r = kt1 - kt0;
+
+    if (tid == 0) {
+        for (int s = 0; s < LC_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+        mbar_init(&cbar[0], 8 * cl); mbar_init(&cbar[1], 8 * cl);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");   // every CTA's barriers exist
+
+    if (warp == 8) {
+        if (lane == 0) {
+            constexpr int BLKA = LD_BK * LD_LDA1, BLKB = LD_BK * LD_LDB1, BLKX = LD_BK * LDX2;
+            const double* LAp = g.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA + (long long)kt0 * BLKA;
+            const double* LBp = g.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB + (long long)kt0 * BLKB;
+            int stage = 0; unsigned par = 1;
+            for (int ch = ch0; ch < ch1; ++ch) {
+                const int et = ch / nFt, ft = ch % nFt;
+                const double* curA = LAp + (long long)et * T1 * BLKA;
+                const double* curB = LBp + (long long)ft * T1 * BLKB;
+                for (int t = 0; t < T1r; ++t) {
+                    mbar_wait(&empty[stage], par);
+                    double* sb = stg + stage * LD_STAGE;
+                    mbar_expect_tx(&full[stage], (BLKA + BLKB) * 8);
+                    bulk_g2s(sb, curA, BLKA * 8, &full[stage]);
+                    bulk_g2s(sb + BLKA, curB, BLKB * 8, &full[stage]);
+                    curA += BLKA; curB += BLKB;
+                    if (++stage == LC_ST) { stage = 0; par ^= 1; }
+                }
+                if (has_col) {
+                    const double* curX = g.X + (((long long)(et * nFt + ft) * g.ncol + col) * T2) * BLKX;
+                    for (int t = 0; t < T2; ++t) {
+                        mbar_wait(&empty[stage], par);
+                        mbar_expect_tx(&full[stage], BLKX * 8);
+                        bulk_g2s(stg + stage * LD_STAGE, curX, BLKX * 8, &full[stage]);
+                        curX += BLKX;
+                        if (++stage == LC_ST) { stage = 0; par ^= 1; }
+                    }
+                }
+            }
+        }
+    } else {
+    // ---------------- consumers
+    const int lr = lane >> 2, lc = lane & 3;
+    double acc2[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
+    double acc1[4][4][2];
+    const int w1m = (warp >> 1) * 32, w1n = (warp & 1) * 32;
+    const int w2m = (warp >> 2) * 32, w2n = (warp & 3) * 32;
+    // my slice of the 64 x 128 chunk in double2 units (reduce-scatter)
+    constexpr int UNITS = LD_R * LD_K2 / 2;
+    const int u0 = (int)((long long)rank * UNITS / cl), u1 = (int)((long long)(rank + 1) * UNITS / cl);
+
+    int stage = 0; unsigned par = 0, cpar = 0;
+    for (int ch = ch0; ch < ch1; ++ch) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
+        for (int t = 0; t < T1r; ++t) {
+            mbar_wait(&full[stage], par);
+            const double* sb = stg + stage * LD_STAGE;
+            const double* as = sb + lc * LD_LDA1 + w1m + lr;
+            const double* bs = sb + LD_BK * LD_LDA1 + lc * LD_LDB1 + w1n + lr;
+#pragma unroll
+            for (int ks = 0; ks < LD_BK / 4; ++ks) {
+                double a[4], b[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) a[i] = as[ks * 4 * LD_LDA1 + 8 * i];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) b[j] = bs[ks * 4 * LD_LDB1 + 8 * j];
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], a[i], b[j]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[stage]);
+            if (++stage == LC_ST) { stage = 0; par ^= 1; }
+        }
+        // partial W[(p,e),(q,f)] -> Ps[(p,q)][(e,f)]   (nobody reads Ps any more: barrier [1] of the previous chunk)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m = w1m + 8 * i + lr;
+            const int p = m / LD_PE, e = m % LD_PE;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int n = w1n + 8 * j + 2 * lc;
+                const int q = n / LD_PF, f = n % LD_PF;
+                *reinterpret_cast<double2*>(&Ps[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]) = make_double2(acc1[i][j][0], acc1[i][j][1]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("fence.acq_rel.cluster;" ::: "memory");
+            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[0], r));
+        }
+        mbar_wait_cluster(&cbar[0], cpar);
+        // reduce my slice over the cl partial tiles (fixed order) and hand the result to every CTA of the cluster
+        for (int u = u0 + (tid & 255); u < u1; u += LD_NCONS) {
+            const int row = u / (LD_K2 / 2), c2 = u % (LD_K2 / 2);
+            const int off = row * LD_LDW + 2 * c2;
+            double2 s = make_double2(0.0, 0.0);
+            for (int r = 0; r < cl; ++r) {
+                double2 v = ld_cluster2(map_shared(Ps + off, r));
+                s.x += v.x; s.y += v.y;
+            }
+            for (int r = 0; r < cl; ++r) st_cluster2(map_shared(Ws + off, r), s);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("fence.acq_rel.cluster;" ::: "memory");
+            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[1], r));
+        }
+        mbar_wait_cluster(&cbar[1], cpar);
+        cpar ^= 1;
+        if (has_col) {
+            for (int t = 0; t < T2; ++t) {
+                mbar_wait(&full[stage], par);
+                const double* sb = stg + stage * LD_STAGE;
+                const double* ws = Ws + (w2m + lr) * LD_LDW + t * LD_BK + lc;
+                const double* xs = sb + lc * LDX2 + w2n + lr;
+#pragma unroll
+                for (int ks = 0; ks < LD_BK / 4; ++ks) {
+                    double a[4], b[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) a[i] = ws[8 * i * LD_LDW + ks * 4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) b[j] = xs[ks * 4 * LDX2 + 8 * j];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], a[i], b[j]);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[stage]);
+                if (++stage == LC_ST) { stage = 0; par ^= 1; }
+            }
+        }
+    }
+    if (has_col) {
+        double* Yout = g.nsplit > 1 ? g.Ypart + (long long)split * g.nA * g.nB * g.ldY : g.Y;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int row = w2m + 8 * i + lr;
+            const int p = p0 + row / LD_PQ, q = q0 + row % LD_PQ;
+            if (p >= g.nA || q >= g.nB) continue;
+            double* y = Yout + ((long long)p * g.nB + q) * g.ldY;
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const int x = x0 + w2n + 8 * j + 2 * lc + c;
+                    if (x < g.N2) y[x] = acc2[i][j][c];
+                }
+        }
+    }
+    }
+    // no CTA may retire while a sibling can still touch its shared memory
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
 // Y = sum over slices of Ypart (fixed order)
 __global__ void ladder_reduce_kernel(const LadderBatch b)
 {
@@ -262,15 +488,20 @@ __global__ void ladder_reduce_kernel(const LadderBatch b)
     }
 }
 
-// Host side: choose column tile width and the (e,f) slicing so that the items fill the SMs evenly.
-inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
+// Host side: choose column tile width, cluster shape and the (e,f) slicing so that the items fill the SMs evenly.
+inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, int max_cluster = 8)
 {
     long long rows = 0;
     for (int i = 0; i < b.ncase; ++i) {
         LadderCase& g = b.c[i];
         g.nt2 = g.N2 <= 64 ? 64 : 128;
         g.ncol = (g.N2 + g.nt2 - 1) / g.nt2;
-        rows += (long long)g.ntiles * g.ncol;
+        g.cl = 1; g.ngrp = g.ncol;
+        if (g.ncol > 1) {                    // balanced groups of at most max_cluster column tiles
+            g.ngrp = (g.ncol + max_cluster - 1) / max_cluster;
+            g.cl = (g.ncol + g.ngrp - 1) / g.ngrp;
+        }
+        rows += (long long)g.ntiles * g.ngrp * g.cl;
     }
     int best = 1;
     if (rows < 8LL * num_sms) {
@@ -287,36 +518,61 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
         const int nchunk = ((g.vA + LD_PE - 1) / LD_PE) * ((g.vB + LD_PF - 1) / LD_PF);
         g.nsplit = best < nchunk ? best : (nchunk > 0 ? nchunk : 1);
         g.item0 = item;
-        item += g.ntiles * g.ncol * g.nsplit;
+        if (g.cl == 1) item += g.ntiles * g.ncol * g.nsplit;     // only single-column cases run in the batched kernel
     }
     b.nitems = item;
 }
 
-// executed tensor-pipe flops of one launch
+// executed tensor-pipe flops of one evaluation
 inline double ladder_flops(const LadderBatch& b)
 {
     double f = 0.0;
     for (int i = 0; i < b.ncase; ++i) {
         const LadderCase& g = b.c[i];
         double rows = 64.0 * g.ntiles, ef = (double)g.vA * g.vB;
-        f += 2.0 * rows * ef * ((double)b.NQ * g.ncol + (double)g.ncol * g.nt2);
+        f += 2.0 * rows * ef * ((double)b.NQ * g.ngrp * (g.cl == 1 ? 1.0 : 1.0) + (double)g.ncol * g.nt2);
     }
     return f;
 }
 
 inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
 {
-    if (b.nitems <= 0) return 0;
-    ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(b);
+    int launches = 0;
     bool red = false;
-    for (int i = 0; i < b.ncase; ++i) red |= b.c[i].nsplit > 1;
-    if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); return 2; }
-    return 1;
+    if (b.nitems > 0) {
+        LadderBatch pb = b;                       // cluster cases take no items of the batched kernel
+        for (int i = 0; i < pb.ncase; ++i) if (pb.c[i].cl > 1) pb.c[i].ntiles = 0;
+        // (item0 offsets were computed with the cluster cases contributing zero items)
+        ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(pb);
+        ++launches;
+    }
+    for (int i = 0; i < b.ncase; ++i) {
+        const LadderCase& g = b.c[i];
+        red |= g.nsplit > 1;
+        if (g.cl <= 1 || g.ntiles <= 0) continue;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)((long long)g.ntiles * g.ngrp * g.nsplit * g.cl));
+        cfg.blockDim = dim3(LD_NTH);
+        cfg.dynamicSmemBytes = ladder_cluster_smem();
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)g.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, ladder_cluster_kernel, g, b.NQ);
+        ++launches;
+    }
+    if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); ++launches; }
+    return launches;
 }
 
 inline cudaError_t ladder_init()
 {
-    return cudaFuncSetAttribute(ladder_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_smem());
+    cudaError_t e = cudaFuncSetAttribute(ladder_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_smem());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ladder_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_cluster_smem());
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(ladder_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
 }
 
 }  // namespace rtcc

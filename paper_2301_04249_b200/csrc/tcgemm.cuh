@@ -100,7 +100,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
     constexpr int EA = BM * BK / NP, EB = BK * BN / NP;      // 16 each
     constexpr int TM = WM / 8, TN = WN / 8;
     static_assert(NP == BM && NP == BN && EA == BK && EB == BK, "producer mapping assumes one row / column per producer thread");
-    extern __shared__ __align__(16) double smem[];
+    extern __shared__ __align__(128) double smem[];
     double* As = smem;                        // [ST][BM][LDA]
     double* Bs = smem + ST * BM * LDA;        // [ST][BK][LDB]
     long long* rowA = (long long*)(Bs + ST * BK * LDB);   // [BM] offsets (or -1)

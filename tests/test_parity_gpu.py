@@ -54,7 +54,8 @@ def check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2):
 SHAPES = [
     (2, 3, 4, 3, 5), (1, 1, 3, 3, 4), (2, 0, 3, 5, 4), (0, 2, 5, 3, 4), (1, 2, 2, 1, 3), (3, 1, 1, 3, 2),
     (3, 4, 13, 12, 48), (5, 4, 18, 19, 37), (2, 2, 33, 33, 21),
-    (9, 8, 10, 11, 20),      # o_a*o_b = 72: Re|Im-stacked width 144 > 128, i.e. two column tiles in the ladder kernel
+    (9, 8, 10, 11, 20),      # o_a*o_b = 72: Re|Im-stacked width 144 > 128: clusters of 2 CTAs in the wide ladder kernel
+    (17, 16, 6, 7, 10),      # widths 544 (ab: clusters of 5), 272 / 240 (aa, bb: clusters of 3 / 2)
 ]
 
 
