@@ -299,6 +299,71 @@ __device__ __forceinline__ double block_max(double v, double* sh)
     return r;
 }
 
+// Fused T1 dressing for problems whose n x n Cholesky slice fits in shared memory (one CTA per Cholesky vector, both
+// spins):  L~^Q = (1 - T) L^Q (1 + T)  and  gamma^Q = sum_s sum_ie L^Q_ie t_i^e.  Replaces the
+// copy + two skinny GEMMs per spin of the general path; same arithmetic, fixed summation order.
+struct DressArgs { const double* L[2]; double* Lt[2]; const double* t1r; double* gam; };
+__global__ void __launch_bounds__(256) k_dress(Dims d, DressArgs A)
+{
+    extern __shared__ double sm[];
+    const int n = d.n, ld = n | 1, Q = blockIdx.x, tid = threadIdx.x;
+    const long long nn = (long long)n * n, plane = (long long)d.NQ * nn;
+    __shared__ double red[32];
+    double gr = 0.0, gi = 0.0;
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        double* Ls = sm;                       // [n][ld]
+        double* tr = Ls + (size_t)n * ld;      // [o][v]
+        double* ti = tr + (size_t)o * v;
+        double* Br = ti + (size_t)o * v;       // [n][o]   (L T)[p][i] = sum_e L[p][o+e] t_i^e
+        double* Bi = Br + (size_t)n * o;
+        __syncthreads();
+        const double* Lg = A.L[s] + Q * nn;
+        for (int x = tid; x < n * n; x += 256) Ls[(x / n) * ld + x % n] = Lg[x];
+        for (int x = tid; x < o * v; x += 256) { tr[x] = A.t1r[off1 + x]; ti[x] = A.t1r[d.n1 + off1 + x]; }
+        __syncthreads();
+        for (int x = tid; x < n * o; x += 256) {
+            const int p = x / o, i = x - p * o;
+            double ar = 0.0, ai = 0.0;
+            for (int e = 0; e < v; ++e) { const double l = Ls[p * ld + o + e]; ar += l * tr[i * v + e]; ai += l * ti[i * v + e]; }
+            Br[x] = ar; Bi[x] = ai;
+        }
+        for (int x = tid; x < o * v; x += 256) { const int i = x / v, e = x - i * v; const double l = Ls[i * ld + o + e]; gr += l * tr[x]; gi += l * ti[x]; }
+        __syncthreads();
+        double* Or = A.Lt[s] + Q * nn;
+        double* Oi = Or + plane;
+        for (int x = tid; x < n * n; x += 256) {
+            const int p = x / n, q = x - p * n;
+            double vr = Ls[p * ld + q], vi = 0.0;
+            if (q < o) { vr += Br[p * o + q]; vi = Bi[p * o + q]; }
+            if (p >= o) {                      // row a: subtract sum_m t_m^a (L Y)[m][q]
+                const int a = p - o;
+                for (int m = 0; m < o; ++m) {
+                    double yr = Ls[m * ld + q], yi = 0.0;
+                    if (q < o) { yr += Br[m * o + q]; yi = Bi[m * o + q]; }
+                    const double xr = tr[m * v + a], xi = ti[m * v + a];
+                    vr -= xr * yr - xi * yi;
+                    vi -= xr * yi + xi * yr;
+                }
+            }
+            Or[x] = vr; Oi[x] = vi;
+        }
+    }
+    const double a = block_sum(gr, red);
+    const double b = block_sum(gi, red);
+    if (tid == 0) { A.gam[Q] = a; A.gam[d.NQ + Q] = b; }
+}
+inline size_t dress_smem(const Dims& d)
+{
+    size_t m = 0;
+    for (int s = 0; s < 2; ++s) {
+        size_t x = (size_t)d.n * (d.n | 1) + 2 * (size_t)d.o[s] * d.v[s] + 2 * (size_t)d.n * d.o[s];
+        if (x > m) m = x;
+    }
+    return m * sizeof(double);
+}
+
 struct EnergyArgs {
     const double* L[2]; const double* Lt[2]; const double* fock[2];   // bare vectors, dressed vectors (planar), bare Fock
     const double* t1r; const double* Mq; const double* gam; double* partial;   // partial[RED_BLOCKS][2]

@@ -566,6 +566,28 @@ inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
     return launches;
 }
 
+// largest cluster size (<= 16) that can actually be co-scheduled with the wide kernel's resources on this device
+inline int ladder_max_cluster()
+{
+    static int cached = 0;
+    if (cached) return cached;
+    int best = 1;
+    for (int cl = 16; cl >= 2; --cl) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)cl * 8); cfg.blockDim = dim3(LD_NTH); cfg.dynamicSmemBytes = ladder_cluster_smem();
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, ladder_cluster_kernel, &cfg) == cudaSuccess && n > 0) { best = cl; break; }
+        cudaGetLastError();
+    }
+    if (const char* e = getenv("RTCC_MAX_CLUSTER")) { int v = atoi(e); if (v >= 1 && v < best) best = v; }
+    cached = best;
+    return best;
+}
+
 inline cudaError_t ladder_init()
 {
     cudaError_t e = cudaFuncSetAttribute(ladder_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_smem());

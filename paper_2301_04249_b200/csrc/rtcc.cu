@@ -62,6 +62,7 @@ struct rtcc_ctx {
     int timing = 0; cudaEvent_t ev[2]{}; double lad_ms = 0, lad_flops = 0, lad_model = 0;
     cudaGraphExec_t graph = nullptr;
     bool capturing = false;
+    bool fused_dress = false;
 };
 
 namespace {
@@ -158,8 +159,17 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
 
     if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
 
-    // ---- 2. T1-dressed Cholesky vectors  L~^Q = (1-T) L^Q (1+T)
+    // ---- 2+3. T1-dressed Cholesky vectors and gamma: one fused kernel when an n x n slice fits in shared memory
     c->sec = 2;
+    if (c->fused_dress) {
+        DressArgs da;
+        for (int s = 0; s < 2; ++s) { da.L[s] = c->L[s]; da.Lt[s] = c->Lt[s]; }
+        da.t1r = c->t1r; da.gam = c->gam;
+        k_dress<<<NQ, 256, dress_smem(d), ST>>>(d, da);
+        c->launches++;
+        if (par) CK(cudaEventRecord(c->evs[1], c->S[0]));     // evs[1]: dressed vectors ready
+    } else {
+    // ---- 2. (general path) T1-dressed Cholesky vectors  L~^Q = (1-T) L^Q (1+T)
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -189,7 +199,6 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     if (par) CK(cudaEventRecord(c->evs[1], c->S[0]));     // evs[1]: dressed vectors ready
 
     // ---- 3. gamma^Q = sum_ie L^Q_ie t_i^e (both spins)
-    c->sec = 3;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -200,6 +209,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         ops_rc(g, c->L[s] + o, c->t1r + off1, n1, c->gam, NQ);
         g.beta = s ? 1.0 : 0.0;
         run(c, g);
+    }
+
     }
 
     // ---- 4. M^Q_ia = sum_me L^Q_me t_im^ae over the spin-conserving pair space
@@ -713,6 +724,10 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
         CKC(tcgemm_init());
         CKC(ladder_init());
+        if (dress_smem(d) <= 200 * 1024 && !getenv("RTCC_NO_FUSED")) {
+            CKC(cudaFuncSetAttribute(k_dress, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dress_smem(d)));
+            c->fused_dress = true;
+        }
         CKC(cudaEventCreate(&c->ev[0]));
         CKC(cudaEventCreate(&c->ev[1]));
         {   // helper branches: everything latency-bound outranks the SM-filling ladder branch (aux[2] = S[3])
@@ -849,7 +864,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
-            ladder_plan(B, c->num_sms, 8);
+            ladder_plan(B, c->num_sms, 8, ladder_max_cluster());
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;
