@@ -512,6 +512,7 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, int max_clus
             if (eff > beff + 0.02) { beff = eff; best = S; }
         }
     }
+    if (const char* e = getenv("RTCC_LADDER_SPLIT")) { int v = atoi(e); if (v >= 1) best = v; }   // tuning knob
     int item = 0;
     for (int i = 0; i < b.ncase; ++i) {
         LadderCase& g = b.c[i];
