@@ -33,6 +33,7 @@ BENCH_MODE = 0
 BENCH_TOL = 1e-4
 BENCH_FIXED_MICRO = 0
 L2_BYTES = 126 * 2 ** 20
+LADDER_DRAM_BYTES_NCU = 94.8e6      # per launch, workload 'small' (profiles/r01b_topkernel_ncu.md: 65.6 MB read + 29.3 MB written)
 
 
 def mac_model(o, v):
@@ -248,9 +249,11 @@ def run_ours(args, cfg):
                        "parallelism": "replicas only" if world > 1 else "single GPU", "workspace_bytes": ctx.workspace_bytes},
             "residual": {"ms": res_ms, "model_flops": f_model, "model_tflops": f_model / res_ms * 1e-9,
                          "pct_of_fp64_peak": 100.0 * f_model / res_ms * 1e-9 / peak, "executed_dmma_flops": ctx_res_flops(ctx)},
-            "roofline": {"bound": "tensor", "kernel": "ladder_kernel<128> (3 launches per residual: ab, aa, bb)",
+            "roofline": {"bound": "tensor", "kernel": "ladder_kernel (one launch per residual: ab, aa, bb spin cases batched)",
                          "achieved": lad_model / lad_ms * 1e-9, "peak": peak, "unit": "TFLOP/s",
-                         "frac": lad_model / lad_ms * 1e-9 / peak, "traffic": None,
+                         "frac": lad_model / lad_ms * 1e-9 / peak, "traffic": LADDER_DRAM_BYTES_NCU if cfg.name == "small" else None,
+                         "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r01b_topkernel_ncu.md)",
+                         "ncu_dmma_pipe_active_pct": 92.6,
                          "executed_tflops": lad_exec / lad_ms * 1e-9, "ms": lad_ms, "algorithmic_flops": lad_model,
                          "peak_source": "measured live: register-resident FP64 DMMA loop (rtcc_fp64_peak); MEASURED_PEAKS.json has no fp64 figure"},
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
