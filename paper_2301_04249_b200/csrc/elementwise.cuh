@@ -364,6 +364,251 @@ inline size_t dress_smem(const Dims& d)
     return m * sizeof(double);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Fused small-problem kernels for the dressed Fock matrix, the F intermediates and the singles (SURVEY.md 8(a) a2, a6,
+// a7): sums over the Cholesky index are split into NCH chunks (one CTA each, fixed order inside), the chunk partials
+// are added in fixed order by k_reduce_chunks, and a one-CTA-per-spin kernel finishes.  Same arithmetic as the tcgemm
+// path they replace; used when the per-thread element counts fit (FUSE_MAXE).
+constexpr int FUSE_T = 512, FUSE_MAXE = 12;
+
+__global__ void k_reduce_chunks(const double* __restrict__ in, double* __restrict__ out, int nchunk, long long len)
+{
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < len; x += (long long)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int c = 0; c < nchunk; ++c) s += in[c * len + x];
+        out[x] = s;
+    }
+}
+
+// part[chunk][s][0..3][n*n]: J = sum_Q gamma^Q L^Q (re, im),  Ex = sum_Q sum_i L~^Q_pi L~^Q_iq (re, im)
+__global__ void __launch_bounds__(FUSE_T) k_fock_partial(Dims d, const double* __restrict__ L0, const double* __restrict__ L1,
+                                                         const double* __restrict__ Lt0, const double* __restrict__ Lt1,
+                                                         const double* __restrict__ gam, int nch, double* __restrict__ part)
+{
+    extern __shared__ double sm[];
+    const int s = blockIdx.y, c = blockIdx.x, tid = threadIdx.x;
+    const int n = d.n, o = d.o[s];
+    const long long nn = (long long)n * n, plane = (long long)d.NQ * nn;
+    const double* L = s ? L1 : L0;
+    const double* Lt = s ? Lt1 : Lt0;
+    double* Ar = sm;                 // L~[p][i]   [n][o]
+    double* Ai = Ar + n * o;
+    double* Br = Ai + n * o;         // L~[i][q]   [o][n]
+    double* Bi = Br + o * n;
+    double jr[FUSE_MAXE], ji[FUSE_MAXE], xr[FUSE_MAXE], xi[FUSE_MAXE];
+#pragma unroll
+    for (int k = 0; k < FUSE_MAXE; ++k) jr[k] = ji[k] = xr[k] = xi[k] = 0.0;
+    const int Q0 = (int)((long long)c * d.NQ / nch), Q1 = (int)((long long)(c + 1) * d.NQ / nch);
+    for (int Q = Q0; Q < Q1; ++Q) {
+        __syncthreads();
+        for (int x = tid; x < n * o; x += FUSE_T) {
+            const int p = x / o, i = x - p * o;
+            Ar[x] = Lt[Q * nn + (long long)p * n + i]; Ai[x] = Lt[plane + Q * nn + (long long)p * n + i];
+        }
+        for (int x = tid; x < o * n; x += FUSE_T) { Br[x] = Lt[Q * nn + x]; Bi[x] = Lt[plane + Q * nn + x]; }
+        __syncthreads();
+        const double gr = gam[Q], gi = gam[d.NQ + Q];
+#pragma unroll
+        for (int k = 0; k < FUSE_MAXE; ++k) {
+            const int e = tid + k * FUSE_T;
+            if (e < nn) {
+                const int p = e / n, q = e - p * n;
+                const double l = L[Q * nn + e];
+                jr[k] += gr * l; ji[k] += gi * l;
+                double ar = 0.0, ai = 0.0;
+                for (int i = 0; i < o; ++i) {
+                    const double pr = Ar[p * o + i], pi = Ai[p * o + i], qr = Br[i * n + q], qi = Bi[i * n + q];
+                    ar += pr * qr - pi * qi; ai += pr * qi + pi * qr;
+                }
+                xr[k] += ar; xi[k] += ai;
+            }
+        }
+    }
+    double* out = part + ((long long)c * 2 + s) * 4 * nn;
+#pragma unroll
+    for (int k = 0; k < FUSE_MAXE; ++k) {
+        const int e = tid + k * FUSE_T;
+        if (e < nn) { out[e] = jr[k]; out[nn + e] = ji[k]; out[2 * nn + e] = xr[k]; out[3 * nn + e] = xi[k]; }
+    }
+}
+
+// f~ = X (Fb + J) Y - Ex   from the reduced sums red[s][0..3][n*n]; writes the planar Ft[s]
+struct FockFinishArgs { const double* Fb[2]; double* Ft[2]; const double* red; const double* t1r; };
+__global__ void __launch_bounds__(FUSE_T) k_fock_finish(Dims d, FockFinishArgs A)
+{
+    extern __shared__ double sm[];
+    const int s = blockIdx.x, tid = threadIdx.x;
+    const int n = d.n, o = d.o[s], v = d.v[s];
+    const long long nn = (long long)n * n, off1 = s ? d.n1a : 0;
+    double* Fr = sm;                 // F0 = Fb + J   [n][n]
+    double* Fi = Fr + nn;
+    double* tr = Fi + nn;            // [o][v]
+    double* ti = tr + o * v;
+    double* Gr = ti + o * v;         // (F0 T)[p][i]  [n][o]
+    double* Gi = Gr + n * o;
+    const double* red = A.red + (long long)s * 4 * nn;
+    for (int x = tid; x < nn; x += FUSE_T) { Fr[x] = A.Fb[s][x] + red[x]; Fi[x] = red[nn + x]; }
+    for (int x = tid; x < o * v; x += FUSE_T) { tr[x] = A.t1r[off1 + x]; ti[x] = A.t1r[d.n1 + off1 + x]; }
+    __syncthreads();
+    for (int x = tid; x < n * o; x += FUSE_T) {
+        const int p = x / o, i = x - p * o;
+        double ar = 0.0, ai = 0.0;
+        for (int e = 0; e < v; ++e) {
+            const double fr = Fr[p * n + o + e], fi = Fi[p * n + o + e], xr = tr[i * v + e], xi = ti[i * v + e];
+            ar += fr * xr - fi * xi; ai += fr * xi + fi * xr;
+        }
+        Gr[x] = ar; Gi[x] = ai;
+    }
+    __syncthreads();
+    for (int x = tid; x < n * o; x += FUSE_T) { const int p = x / o, i = x - p * o; Fr[p * n + i] += Gr[x]; Fi[p * n + i] += Gi[x]; }
+    __syncthreads();
+    double* Or = A.Ft[s];
+    double* Oi = Or + nn;
+    for (int x = tid; x < nn; x += FUSE_T) {
+        const int p = x / n, q = x - p * n;
+        double vr = Fr[x], vi = Fi[x];
+        if (p >= o) {
+            const int a = p - o;
+            for (int m = 0; m < o; ++m) {
+                const double xr = tr[m * v + a], xi = ti[m * v + a], yr = Fr[m * n + q], yi = Fi[m * n + q];
+                vr -= xr * yr - xi * yi; vi -= xr * yi + xi * yr;
+            }
+        }
+        Or[x] = vr - red[2 * nn + x]; Oi[x] = vi - red[3 * nn + x];
+    }
+}
+
+// part[chunk][s][pl][SZ]:  [0, v*v): -sum_Q,m L_me M_ma  (a,e);  then o*o: +sum_Q,e L_me M_ie (m,i);
+//                          then o*v: -sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af  (i,a)
+__global__ void __launch_bounds__(FUSE_T) k_postm_partial(Dims d, const double* __restrict__ L0, const double* __restrict__ L1,
+                                                          const double* __restrict__ Lt0, const double* __restrict__ Lt1,
+                                                          const double* __restrict__ Mq, int nch, long long SZ, double* __restrict__ part)
+{
+    extern __shared__ double sm[];
+    const int s = blockIdx.y, c = blockIdx.x, tid = threadIdx.x;
+    const int n = d.n, o = d.o[s], v = d.v[s];
+    const long long nn = (long long)n * n, plane = (long long)d.NQ * nn, off1 = s ? d.n1a : 0, ld1 = 2LL * d.n1;
+    const double* L = s ? L1 : L0;
+    const double* Lt = s ? Lt1 : Lt0;
+    double* Lov = sm;                    // [o][v]
+    double* Mr = Lov + o * v;            // [o][v]
+    double* Mi = Mr + o * v;
+    double* Or_ = Mi + o * v;            // L~oo [o][o]
+    double* Oi_ = Or_ + o * o;
+    double* Vr = Oi_ + o * o;            // L~vv [v][v]
+    double* Vi = Vr + v * v;
+    double far_[FUSE_MAXE], fai[FUSE_MAXE], fmr = 0.0, fmi = 0.0, r1r[2] = {0.0, 0.0}, r1i[2] = {0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < FUSE_MAXE; ++k) far_[k] = fai[k] = 0.0;
+    const int Q0 = (int)((long long)c * d.NQ / nch), Q1 = (int)((long long)(c + 1) * d.NQ / nch);
+    for (int Q = Q0; Q < Q1; ++Q) {
+        __syncthreads();
+        for (int x = tid; x < o * v; x += FUSE_T) {
+            const int m = x / v, e = x - m * v;
+            Lov[x] = L[Q * nn + (long long)m * n + o + e];
+            Mr[x] = Mq[Q * ld1 + off1 + x]; Mi[x] = Mq[Q * ld1 + d.n1 + off1 + x];
+        }
+        for (int x = tid; x < o * o; x += FUSE_T) {
+            const int m = x / o, i = x - m * o;
+            Or_[x] = Lt[Q * nn + (long long)m * n + i]; Oi_[x] = Lt[plane + Q * nn + (long long)m * n + i];
+        }
+        for (int x = tid; x < v * v; x += FUSE_T) {
+            const int a = x / v, f = x - a * v;
+            Vr[x] = Lt[Q * nn + (long long)(o + a) * n + o + f]; Vi[x] = Lt[plane + Q * nn + (long long)(o + a) * n + o + f];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < FUSE_MAXE; ++k) {
+            const int x = tid + k * FUSE_T;
+            if (x < v * v) {
+                const int a = x / v, e = x - a * v;
+                double ar = 0.0, ai = 0.0;
+                for (int m = 0; m < o; ++m) { const double l = Lov[m * v + e]; ar += l * Mr[m * v + a]; ai += l * Mi[m * v + a]; }
+                far_[k] -= ar; fai[k] -= ai;
+            }
+        }
+        if (tid < o * o) {
+            const int m = tid / o, i = tid - m * o;
+            double ar = 0.0, ai = 0.0;
+            for (int e = 0; e < v; ++e) { const double l = Lov[m * v + e]; ar += l * Mr[i * v + e]; ai += l * Mi[i * v + e]; }
+            fmr += ar; fmi += ai;
+        }
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int x = tid + k * FUSE_T;
+            if (x < o * v) {
+                const int i = x / v, a = x - i * v;
+                double ar = 0.0, ai = 0.0;
+                for (int m = 0; m < o; ++m) {
+                    const double mr = Mr[m * v + a], mi = Mi[m * v + a], lr = Or_[m * o + i], li = Oi_[m * o + i];
+                    ar -= mr * lr - mi * li; ai -= mr * li + mi * lr;
+                }
+                for (int f = 0; f < v; ++f) {
+                    const double mr = Mr[i * v + f], mi = Mi[i * v + f], lr = Vr[a * v + f], li = Vi[a * v + f];
+                    ar += mr * lr - mi * li; ai += mr * li + mi * lr;
+                }
+                r1r[k] += ar; r1i[k] += ai;
+            }
+        }
+    }
+    double* out = part + ((long long)c * 2 + s) * 2 * SZ;
+#pragma unroll
+    for (int k = 0; k < FUSE_MAXE; ++k) {
+        const int x = tid + k * FUSE_T;
+        if (x < v * v) { out[x] = far_[k]; out[SZ + x] = fai[k]; }
+    }
+    if (tid < o * o) { out[v * v + tid] = fmr; out[SZ + v * v + tid] = fmi; }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const int x = tid + k * FUSE_T;
+        if (x < o * v) { out[v * v + o * o + x] = r1r[k]; out[SZ + v * v + o * o + x] = r1i[k]; }
+    }
+}
+
+// Ft vv += F_ae part, Ft oo += F_mi part, r1buf += singles part   (red[s][pl][SZ])
+__global__ void k_postm_finish(Dims d, const double* __restrict__ red, long long SZ, double* __restrict__ Ft0, double* __restrict__ Ft1,
+                               double* __restrict__ r1buf)
+{
+    const int n = d.n;
+    const long long nn = (long long)n * n;
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = s ? d.n1a : 0;
+        double* Ft = s ? Ft1 : Ft0;
+        const long long tot = (long long)v * v + o * o + o * v;
+        for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < 2 * tot; x += (long long)gridDim.x * blockDim.x) {
+            const int pl = x >= tot; const long long y = pl ? x - tot : x;
+            const double val = red[((long long)s * 2 + pl) * SZ + y];
+            if (y < (long long)v * v) { const int a = (int)(y / v), e = (int)(y - (long long)a * v); Ft[pl * nn + (long long)(o + a) * n + o + e] += val; }
+            else if (y < (long long)v * v + o * o) { const long long z = y - (long long)v * v; const int m = (int)(z / o), i = (int)(z - (long long)m * o); Ft[pl * nn + (long long)m * n + i] += val; }
+            else { const long long z = y - (long long)v * v - o * o; r1buf[pl * (long long)d.n1 + off1 + z] += val; }
+        }
+    }
+}
+
+// r1buf[x] = sum_(s,m,e) Tsc[x][(m,e)] f~_me     (one warp per row; complex x complex)
+__global__ void __launch_bounds__(256) k_tsc_matvec(Dims d, const double* __restrict__ Tsc, const double* __restrict__ Ft0,
+                                                     const double* __restrict__ Ft1, double* __restrict__ r1buf)
+{
+    const int n = d.n, n1 = d.n1, lane = threadIdx.x & 31;
+    const long long nn = (long long)n * n;
+    const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (row >= n1) return;
+    const double* Tr = Tsc + (long long)row * 2 * n1;
+    const double* Ti = Tr + n1;
+    double ar = 0.0, ai = 0.0;
+    for (int c = lane; c < n1; c += 32) {
+        const int s = c >= d.n1a; const int cc = s ? c - d.n1a : c;
+        const int m = cc / d.v[s], e = cc - m * d.v[s];
+        const double* F = s ? Ft1 : Ft0;
+        const double fr = F[(long long)m * n + d.o[s] + e], fi = F[nn + (long long)m * n + d.o[s] + e];
+        const double tr = Tr[c], ti = Ti[c];
+        ar += tr * fr - ti * fi; ai += tr * fi + ti * fr;
+    }
+    for (int o = 16; o > 0; o >>= 1) { ar += __shfl_down_sync(0xffffffffu, ar, o); ai += __shfl_down_sync(0xffffffffu, ai, o); }
+    if (lane == 0) { r1buf[row] = ar; r1buf[n1 + row] = ai; }
+}
+
 struct EnergyArgs {
     const double* L[2]; const double* Lt[2]; const double* fock[2];   // bare vectors, dressed vectors (planar), bare Fock
     const double* t1r; const double* Mq; const double* gam; double* partial;   // partial[RED_BLOCKS][2]

@@ -62,7 +62,9 @@ struct rtcc_ctx {
     int timing = 0; cudaEvent_t ev[2]{}; double lad_ms = 0, lad_flops = 0, lad_model = 0;
     cudaGraphExec_t graph = nullptr;
     bool capturing = false;
-    bool fused_dress = false;
+    bool fused_dress = false, fused_fock = false;
+    int fuse_nch = 74; long long fuse_sz = 0; size_t smem_fockp = 0, smem_fockf = 0, smem_postp = 0;
+    double *fockPart = nullptr, *fockRed = nullptr, *postPart = nullptr, *postRed = nullptr;
 };
 
 namespace {
@@ -240,8 +242,28 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         c->launches += 2;
     }
 
-    // ---- 6. dressed Fock  f~ = X (f + K_bare + sum_Q gamma^Q L^Q) Y - sum_Q,i L~^Q_pi L~^Q_iq
+    // ---- 6+7 (fused path for small problems): dressed Fock, F intermediates and singles in seven launches on branch 4
     c->sec = 6;
+    if (c->fused_fock) {
+        const int nch = c->fuse_nch;
+        const long long SZ = c->fuse_sz;
+        BR(4);
+        WAITEV(4, 1);
+        k_fock_partial<<<dim3(nch, 2), FUSE_T, c->smem_fockp, ST>>>(d, c->L[0], c->L[1], c->Lt[0], c->Lt[1], c->gam, nch, c->fockPart);
+        k_reduce_chunks<<<c->num_sms, 256, 0, ST>>>(c->fockPart, c->fockRed, nch, 8 * nn);
+        FockFinishArgs fa;
+        for (int s = 0; s < 2; ++s) { fa.Fb[s] = c->Fb[s]; fa.Ft[s] = c->Ft[s]; }
+        fa.red = c->fockRed; fa.t1r = c->t1r;
+        k_fock_finish<<<2, FUSE_T, c->smem_fockf, ST>>>(d, fa);
+        k_tsc_matvec<<<(n1 + 7) / 8, 256, 0, ST>>>(d, c->Tsc, c->Ft[0], c->Ft[1], c->r1buf);
+        WAITEV(4, 6);
+        k_postm_partial<<<dim3(nch, 2), FUSE_T, c->smem_postp, ST>>>(d, c->L[0], c->L[1], c->Lt[0], c->Lt[1], c->Mq, nch, SZ, c->postPart);
+        k_reduce_chunks<<<c->num_sms, 256, 0, ST>>>(c->postPart, c->postRed, nch, 4 * SZ);
+        k_postm_finish<<<32, 256, 0, ST>>>(d, c->postRed, SZ, c->Ft[0], c->Ft[1], c->r1buf);
+        c->launches += 7;
+        if (par) { CK(cudaEventRecord(c->evs[2], c->S[4])); CK(cudaEventRecord(c->evs[7], c->S[4])); }
+    } else {
+    // ---- 6. dressed Fock  f~ = X (f + K_bare + sum_Q gamma^Q L^Q) Y - sum_Q,i L~^Q_pi L~^Q_iq
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -311,7 +333,6 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     WAITEV(4, 2);                                         // singles stay on branch 4
 
     // ---- 7. singles:  r1 = sum_me t_im^ae f~_me - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af   (+ f~_ai at assembly)
-    c->sec = 7;
     for (int s = 0; s < 2; ++s) {
         const int o = d.o[s], v = d.v[s];
         const long long off1 = s ? d.n1a : 0;
@@ -345,6 +366,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             g.beta = 1.0;
             run(c, g);
         }
+    }
+
     }
 
     // ---- 8. driver + Coulomb ring channel:  Zsc = 1/2 N^T N,  N^Q_ia = L~^Q_ai + M^Q_ia
@@ -727,6 +750,20 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         if (dress_smem(d) <= 200 * 1024 && !getenv("RTCC_NO_FUSED")) {
             CKC(cudaFuncSetAttribute(k_dress, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dress_smem(d)));
             c->fused_dress = true;
+            // dressed Fock / F / singles fused kernels: per-thread element counts and shared memory must fit
+            const int om = d.o[0] > d.o[1] ? d.o[0] : d.o[1], vm = d.v[0] > d.v[1] ? d.v[0] : d.v[1];
+            c->smem_fockp = sizeof(double) * 4 * (size_t)n * om;
+            c->smem_fockf = sizeof(double) * (2 * (size_t)nn + 2 * (size_t)om * vm + 2 * (size_t)n * om);
+            c->smem_postp = sizeof(double) * (3 * (size_t)om * vm + 2 * (size_t)om * om + 2 * (size_t)vm * vm);
+            if (nn <= FUSE_MAXE * FUSE_T && (long long)vm * vm <= FUSE_MAXE * FUSE_T && om * om <= FUSE_T && om * vm <= 2 * FUSE_T &&
+                c->smem_fockf <= 200 * 1024 && c->smem_postp <= 200 * 1024) {
+                CKC(cudaFuncSetAttribute(k_fock_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_fockp));
+                CKC(cudaFuncSetAttribute(k_fock_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_fockf));
+                CKC(cudaFuncSetAttribute(k_postm_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_postp));
+                c->fuse_nch = NQ < 74 ? NQ : 74;
+                c->fuse_sz = (long long)vm * vm + (long long)om * om + (long long)om * vm;
+                c->fused_fock = !getenv("RTCC_NO_FUSED_FOCK");
+            }
         }
         CKC(cudaEventCreate(&c->ev[0]));
         CKC(cudaEventCreate(&c->ev[1]));
@@ -785,6 +822,12 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
         DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
         DA(c->Mq, 2LL * NQ * n1, "Mq");
+        if (c->fused_fock) {
+            DA(c->fockPart, (long long)c->fuse_nch * 8 * nn, nullptr);
+            DA(c->fockRed, 8 * nn, nullptr);
+            DA(c->postPart, (long long)c->fuse_nch * 4 * c->fuse_sz, nullptr);
+            DA(c->postRed, 4 * c->fuse_sz, nullptr);
+        }
         DA(c->Nq, 2LL * NQ * n1, "Nq");
         DA(c->gam, 2LL * NQ, "gam");
         DA(c->r1buf, 2LL * n1, "r1buf");

@@ -230,3 +230,19 @@ def test_residual_small_config_full_size_sampled(rtcc, amp_std):
     assert worst <= RTOL * scale, (worst, scale)
     Eo = so.energy()
     assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
+
+
+def test_general_gemm_path_without_fused_small_kernels(rtcc, monkeypatch):
+    """The fused small-problem kernels (k_dress, k_fock_*, k_postm_*) replace tcgemm launches only when a slice fits in
+    shared memory; the general path must give the same residual (it is the one larger configurations run)."""
+    oa, ob, va, vb, K = 5, 4, 18, 19, 37
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=77)
+    d = orc.Dims(oa, ob, va, vb, K)
+    rng = np.random.default_rng(8)
+    t1 = 0.1 * (rng.standard_normal(d.n_t1) + 1j * rng.standard_normal(d.n_t1))
+    t2 = 0.1 * (rng.standard_normal(d.n_t2) + 1j * rng.standard_normal(d.n_t2))
+    monkeypatch.setenv("RTCC_NO_FUSED", "1")
+    check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+    monkeypatch.delenv("RTCC_NO_FUSED")
+    monkeypatch.setenv("RTCC_NO_FUSED_FOCK", "1")
+    check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
