@@ -99,7 +99,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
     constexpr int LDA = BK + 4, LDB = BN + 4;
     constexpr int EA = BM * BK / NP, EB = BK * BN / NP;      // 16 each
     constexpr int TM = WM / 8, TN = WN / 8;
-    static_assert(NP == BM && NP == BN && EA == BK && EB == BK, "producer mapping assumes one row / column per producer thread");
+    static_assert(NP % BM == 0 && NP % BN == 0 && NP % BK == 0, "producer mapping");
     extern __shared__ __align__(128) double smem[];
     double* As = smem;                        // [ST][BM][LDA]
     double* Bs = smem + ST * BM * LDA;        // [ST][BK][LDB]
@@ -149,12 +149,12 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
         if (a_kfast) {
 #pragma unroll
             for (int j = 0; j < EA; ++j) ra[j] = rowA[p / BK + (NP / BK) * j];
-        } else ra[0] = rowA[p];
+        } else ra[0] = rowA[p % BM];
         long long cb[EB];
         if (!b_nfast) {
 #pragma unroll
             for (int j = 0; j < EB; ++j) cb[j] = colB[p / BK + (NP / BK) * j];
-        } else cb[0] = colB[p];
+        } else cb[0] = colB[p % BN];
         int stage = 0; unsigned par = 1;
         for (int t = 0; t < total; ++t) {
             const int ph = t >= nk ? 1 : 0;
@@ -177,40 +177,42 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
             } else {
                 const bool rv = ra[0] >= 0;
                 const double* Ar = A + (rv ? ra[0] : 0);
-                double* d = as + p * LDA;
+                const int kq = (p / BM) * EA;                    // this thread's k sub-range of the tile
+                double* d = as + (p % BM) * LDA + kq;
                 if (k1a) {
-                    const double* s = Ar + (long long)kbase * g.ak_lo;
+                    const double* s = Ar + (long long)(kbase + kq) * g.ak_lo;
 #pragma unroll
                     for (int j = 0; j < EA; ++j) {
-                        const bool v = rv && (kbase + j < g.K);
+                        const bool v = rv && (kbase + kq + j < g.K);
                         cp_async8p(d + j, v ? s : A, v);
                         s += g.ak_lo;
                     }
                 } else {
 #pragma unroll
                     for (int j = 0; j < EA; ++j) {
-                        const bool v = rv && (kbase + j < g.K);
-                        cp_async8p(d + j, v ? Ar + idx2(kbase + j, g.Klo, g.ak_hi, g.ak_lo) : A, v);
+                        const bool v = rv && (kbase + kq + j < g.K);
+                        cp_async8p(d + j, v ? Ar + idx2(kbase + kq + j, g.Klo, g.ak_hi, g.ak_lo) : A, v);
                     }
                 }
             }
             if (b_nfast) {
                 const bool cv = cb[0] >= 0;
                 const double* Bc = B + (cv ? cb[0] : 0);
-                double* d = bs + p;
+                const int kq = (p / BN) * EB;
+                double* d = bs + kq * LDB + p % BN;
                 if (k1b) {
-                    const double* s = Bc + (long long)kbase * g.bk_lo;
+                    const double* s = Bc + (long long)(kbase + kq) * g.bk_lo;
 #pragma unroll
                     for (int j = 0; j < EB; ++j) {
-                        const bool v = cv && (kbase + j < g.K);
+                        const bool v = cv && (kbase + kq + j < g.K);
                         cp_async8p(d + j * LDB, v ? s : B, v);
                         s += g.bk_lo;
                     }
                 } else {
 #pragma unroll
                     for (int j = 0; j < EB; ++j) {
-                        const bool v = cv && (kbase + j < g.K);
-                        cp_async8p(d + j * LDB, v ? Bc + idx2(kbase + j, g.Klo, g.bk_hi, g.bk_lo) : B, v);
+                        const bool v = cv && (kbase + kq + j < g.K);
+                        cp_async8p(d + j * LDB, v ? Bc + idx2(kbase + kq + j, g.Klo, g.bk_hi, g.bk_lo) : B, v);
                     }
                 }
             } else {
@@ -370,7 +372,7 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     if (big) {
         tcgemm_kernel<128, 128, 64, 32><<<grid, 384, tcgemm_smem<128, 128>(), st>>>(g);
     } else {
-        tcgemm_kernel<64, 64, 32, 32><<<grid, 192, tcgemm_smem<64, 64>(), st>>>(g);
+        tcgemm_kernel<64, 64, 16, 32><<<grid, 384, tcgemm_smem<64, 64>(), st>>>(g);
     }
     if (ks > 1) {
         long long tot = (long long)g.M * g.N * nbt;
@@ -387,7 +389,7 @@ inline cudaError_t tcgemm_init()
     cudaError_t e = cudaFuncSetAttribute(tcgemm_kernel<128, 128, 64, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)tcgemm_smem<128, 128>());
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tcgemm_kernel<64, 64, 32, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(tcgemm_kernel<64, 64, 16, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)tcgemm_smem<64, 64>());
 }
 
