@@ -91,6 +91,22 @@ int rtcc_reset_counters(rtcc_ctx* ctx);
 int rtcc_set_timing(rtcc_ctx* ctx, int on);
 int rtcc_ladder_timing(const rtcc_ctx* ctx, double* ms, double* flops, double* model_flops);
 
+/* (N-1)-electron Fock matrix from the Cholesky vectors and the orbital energies of the N-electron reference
+ * (f_pq = eps_p delta_pq - v_pc^qc, c = core-hole spin-orbital; v_pq^rs = <pq||rs>):
+ *   fock[s][p][q] = eps[s][p] delta_pq - sum_Q L[s][Q][p][q] L[cs][Q][c][c] + delta(s,cs) sum_Q L[s][Q][p][c] L[s][Q][c][q]
+ * L [2][n_chol][n][n], eps [2][n], fock [2][n][n] (out); core_spin in {0,1}, 0 <= core_index < n (position of the core
+ * orbital in that spin's orbital order).  flags & RTCC_HOST_PTRS: arrays are host pointers, else device pointers. */
+int rtcc_build_fock(int n, int n_chol, const double* L, const double* eps, int core_spin, int core_index, double* fock,
+                    unsigned flags, void* cuda_stream);
+
+/* Core-hole Green's function and spectral function from a recorded cumulant (PAPER.md:41, :52-56 Eqs. 3-4; :103):
+ *   G(tau_k) = -i exp(-i (eps_c + e_corr) tau_k) exp(C(tau_k)),   tau_k = k dt, k = 0..nt-1
+ *   A(omega) = -(1/pi) Im int_0^T G(tau) exp(i omega tau - eta tau) dtau      (trapezoid rule on the recorded grid;
+ *   the paper does not state its broadening: eta >= 0 is the caller's Lorentzian half width, reading R14)
+ * All pointers are HOST pointers: C [nt][2] (re, im), omega [nw], G [nt][2] out (may be NULL), A [nw] out. */
+int rtcc_spectral_function(int nt, double dt, const double* C, double eps_c, double e_corr, double eta, int nw,
+                           const double* omega, double* G, double* A);
+
 /* Measured FP64 tensor-pipe peak (TFLOP/s) of the current device: register-resident DMMA loop. */
 int rtcc_fp64_peak(double* tflops);
 

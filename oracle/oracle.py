@@ -283,3 +283,40 @@ class Propagator:
         self.time += dt
         self.last_micro = k
         return k
+
+
+# ----------------------------------------------------------------------------- NEXT-3 / NEXT-2
+def build_fock_n1(L, eps, core_spin: int, core_index: int):
+    """(N-1)-electron Fock matrix f_pq = eps_p delta_pq - v_pc^qc, v_pq^rs = <pq||rs>, written
+    out per spin: f^s_pq = eps^s_p delta_pq - (pq|cc) + delta(s, s_c) (pc|cq), (pq|rs) = sum_Q L_pq L_rs.
+    L[2,K,n,n], eps[2,n] -> fock[2,n,n].  Pinned against -<pc||qc> of the spin-orbital tensor (test_fock_n1_*)."""
+    L = np.asarray(L, dtype=np.float64)
+    eps = np.asarray(eps, dtype=np.float64)
+    n = L.shape[2]
+    fock = np.zeros((2, n, n))
+    Lcc = L[core_spin][:, core_index, core_index]
+    for s in range(2):
+        fock[s] = np.diag(eps[s]) - np.einsum("Qpq,Q->pq", L[s], Lcc)
+        if s == core_spin:
+            fock[s] += np.einsum("Qp,Qq->pq", L[s][:, :, core_index], L[s][:, core_index, :])
+    return fock
+
+
+def green_function(C, dt, eps_c, e_corr):
+    """G_c^R(tau_k) = -i exp(-i (eps_c + E_N^corr) tau_k) exp(C(tau_k)), tau_k = k dt >= 0   (Eqs. 3-4)."""
+    C = np.asarray(C, dtype=np.complex128)
+    tau = dt * np.arange(C.size)
+    return -1j * np.exp(-1j * (eps_c + e_corr) * tau) * np.exp(C)
+
+
+def spectral_function(C, dt, eps_c, e_corr, eta, omega):
+    """A_c(omega) = -(1/pi) Im G_c^R(omega), G(omega) = int_0^T G(tau) exp(i omega tau - eta tau) dtau by the
+    trapezoid rule on the recorded grid (reading R14: eta is the caller's Lorentzian half width)."""
+    G = green_function(C, dt, eps_c, e_corr)
+    tau = dt * np.arange(G.size)
+    w = np.full(G.size, dt)
+    w[0] = w[-1] = 0.5 * dt
+    out = np.empty(len(omega))
+    for k, om in enumerate(np.asarray(omega, dtype=np.float64)):
+        out[k] = -np.imag(np.sum(w * G * np.exp((1j * om - eta) * tau))) / np.pi
+    return G, out

@@ -767,6 +767,51 @@ __global__ void k_build_Dn(Dims d, const double* __restrict__ f0, const double* 
     }
 }
 
+// (N-1) Fock matrix, PAPER.md:48 (see include/rtcc.h: rtcc_build_fock)
+__global__ void k_build_fock(int n, int NQ, const double* __restrict__ L, const double* __restrict__ eps, int cs, int ci,
+                             double* __restrict__ fock)
+{
+    const long long nn = (long long)n * n;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < 2 * nn; x += (long long)gridDim.x * blockDim.x) {
+        const int s = (int)(x / nn); const long long r = x - s * nn;
+        const int p = (int)(r / n), q = (int)(r - (long long)p * n);
+        const double* Ls = L + (long long)s * NQ * nn;
+        const double* Lc = L + (long long)cs * NQ * nn;
+        double coul = 0.0, exch = 0.0;
+        for (int Q = 0; Q < NQ; ++Q) {
+            coul += Ls[Q * nn + r] * Lc[Q * nn + (long long)ci * n + ci];
+            if (s == cs) exch += Ls[Q * nn + (long long)p * n + ci] * Ls[Q * nn + (long long)ci * n + q];
+        }
+        fock[x] = (p == q ? eps[s * n + p] : 0.0) - coul + exch;
+    }
+}
+
+// G(tau_k) and A(omega): one block per frequency, fixed-order block reduction (see include/rtcc.h: rtcc_spectral_function)
+__global__ void k_green(int nt, double dt, const double* __restrict__ C, double e0, double* __restrict__ G)
+{
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nt; k += gridDim.x * blockDim.x) {
+        const double tau = k * dt, m = exp(C[2 * k]), ph = C[2 * k + 1] - e0 * tau;      // exp(C) exp(-i e0 tau)
+        const double zr = m * cos(ph), zi = m * sin(ph);
+        G[2 * k] = zi; G[2 * k + 1] = -zr;                                                // times -i
+    }
+}
+__global__ void __launch_bounds__(RED_THREADS) k_spectral(int nt, double dt, const double* __restrict__ G, double eta, int nw,
+                                                           const double* __restrict__ omega, double* __restrict__ A)
+{
+    __shared__ double sh[32];
+    const int w = blockIdx.x;
+    if (w >= nw) return;
+    const double om = omega[w];
+    double acc = 0.0;                      // Im of the integral
+    for (int k = threadIdx.x; k < nt; k += blockDim.x) {
+        const double tau = k * dt, wgt = (k == 0 || k == nt - 1) ? 0.5 * dt : dt, d = exp(-eta * tau);
+        const double c = cos(om * tau), s = sin(om * tau);
+        acc += wgt * d * (G[2 * k] * s + G[2 * k + 1] * c);
+    }
+    const double r = block_sum(acc, sh);
+    if (threadIdx.x == 0) A[w] = -r / 3.14159265358979323846;
+}
+
 // FP64 tensor-pipe peak probe: register-resident DMMA loop (denominator of the contraction roofline)
 __global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters, double seed)
 {

@@ -488,8 +488,50 @@ __global__ void ladder_reduce_kernel(const LadderBatch b)
     }
 }
 
+// SMs that clusters of cl CTAs of the wide kernel can keep busy at once (0: size not schedulable); cached per size
+inline int ladder_cluster_active_sms(int cl, int num_sms)
+{
+    static int tab[17] = {0};
+    static bool done = false;
+    if (!done) {
+        for (int c = 2; c <= 16; ++c) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)c * 64); cfg.blockDim = dim3(LD_NTH); cfg.dynamicSmemBytes = ladder_cluster_smem();
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, ladder_cluster_kernel, &cfg) == cudaSuccess && n > 0) tab[c] = n * c;
+            cudaGetLastError();
+        }
+        done = true;
+    }
+    int a = (cl >= 2 && cl <= 16) ? tab[cl] : 0;
+    return a > num_sms ? num_sms : a;
+}
+// cluster size for ncol column tiles: minimise  groups * (W1 + cl * W2) / active SMs   (W1: building one W chunk,
+// W2: applying it to one column tile); a cluster never spans more column tiles than there are
+inline int ladder_choose_cluster(int ncol, int NQ, int num_sms)
+{
+    int maxc = 16;
+    if (const char* e = getenv("RTCC_MAX_CLUSTER")) { int v = atoi(e); if (v >= 2 && v < maxc) maxc = v; }
+    const double W1 = 128.0 * 64.0 * NQ, W2 = 64.0 * 128.0 * 128.0;
+    int best = 0; double bt = 1e300;
+    for (int cl = 2; cl <= maxc; ++cl) {
+        const int act = ladder_cluster_active_sms(cl, num_sms);
+        if (act <= 0) continue;
+        const int ngrp = (ncol + cl - 1) / cl;
+        const int ceff = (ncol + ngrp - 1) / ngrp;          // balanced groups
+        if (ceff != cl && cl <= ncol) continue;             // evaluate each balanced size once
+        const double t = ngrp * (W1 + ceff * W2) / ladder_cluster_active_sms(ceff, num_sms);
+        if (ladder_cluster_active_sms(ceff, num_sms) > 0 && t < bt) { bt = t; best = ceff; }
+    }
+    return best > 0 ? best : 2;
+}
+
 // Host side: choose column tile width, cluster shape and the (e,f) slicing so that the items fill the SMs evenly.
-inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, int max_cluster = 8)
+inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
 {
     long long rows = 0;
     for (int i = 0; i < b.ncase; ++i) {
@@ -498,8 +540,8 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, int max_clus
         g.ncol = (g.N2 + g.nt2 - 1) / g.nt2;
         g.cl = 1; g.ngrp = g.ncol;
         if (g.ncol > 1) {                    // balanced groups of at most max_cluster column tiles
-            g.ngrp = (g.ncol + max_cluster - 1) / max_cluster;
-            g.cl = (g.ncol + g.ngrp - 1) / g.ngrp;
+            g.cl = ladder_choose_cluster(g.ncol, b.NQ, num_sms);
+            g.ngrp = (g.ncol + g.cl - 1) / g.cl;
         }
         rows += (long long)g.ntiles * g.ngrp * g.cl;
     }
@@ -565,28 +607,6 @@ inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
     }
     if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); ++launches; }
     return launches;
-}
-
-// largest cluster size (<= 16) that can actually be co-scheduled with the wide kernel's resources on this device
-inline int ladder_max_cluster()
-{
-    static int cached = 0;
-    if (cached) return cached;
-    int best = 1;
-    for (int cl = 16; cl >= 2; --cl) {
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)cl * 8); cfg.blockDim = dim3(LD_NTH); cfg.dynamicSmemBytes = ladder_cluster_smem();
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = (unsigned)cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, ladder_cluster_kernel, &cfg) == cudaSuccess && n > 0) { best = cl; break; }
-        cudaGetLastError();
-    }
-    if (const char* e = getenv("RTCC_MAX_CLUSTER")) { int v = atoi(e); if (v >= 1 && v < best) best = v; }
-    cached = best;
-    return best;
 }
 
 inline cudaError_t ladder_init()

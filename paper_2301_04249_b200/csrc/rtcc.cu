@@ -907,7 +907,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
-            ladder_plan(B, c->num_sms, 8, ladder_max_cluster());
+            ladder_plan(B, c->num_sms, 8);
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;
@@ -1149,6 +1149,44 @@ int rtcc_ladder_timing(const rtcc_ctx* c, double* ms, double* flops, double* mod
     if (flops) *flops = c->lad_flops;
     if (model_flops) *model_flops = c->lad_model;
     return RTCC_OK;
+}
+
+int rtcc_build_fock(int n, int NQ, const double* L, const double* eps, int cs, int ci, double* fock, unsigned flags, void* stream)
+{
+    if (n < 1 || NQ < 1 || !L || !eps || !fock || (cs != 0 && cs != 1) || ci < 0 || ci >= n) return RTCC_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long nn = (long long)n * n, nL = 2LL * NQ * nn;
+    const double *dL = L, *de = eps; double* df = fock;
+    double* buf = nullptr;
+    if (flags & RTCC_HOST_PTRS) {
+        if (cudaMalloc(&buf, (size_t)(nL + 2 * n + 2 * nn) * 8) != cudaSuccess) { cudaGetLastError(); return RTCC_ENOMEM; }
+        cudaMemcpyAsync(buf, L, (size_t)nL * 8, cudaMemcpyHostToDevice, st);
+        cudaMemcpyAsync(buf + nL, eps, (size_t)2 * n * 8, cudaMemcpyHostToDevice, st);
+        dL = buf; de = buf + nL; df = buf + nL + 2 * n;
+    }
+    k_build_fock<<<nblk(2 * nn, 148 * 8), 256, 0, st>>>(n, NQ, dL, de, cs, ci, df);
+    if (flags & RTCC_HOST_PTRS) cudaMemcpyAsync(fock, df, (size_t)2 * nn * 8, cudaMemcpyDeviceToHost, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (buf) cudaFree(buf);
+    return e == cudaSuccess ? RTCC_OK : RTCC_ECUDA;
+}
+
+int rtcc_spectral_function(int nt, double dt, const double* C, double eps_c, double e_corr, double eta, int nw,
+                           const double* omega, double* G, double* A)
+{
+    if (nt < 2 || nw < 1 || !C || !omega || !A || !(dt > 0.0) || !(eta >= 0.0) || !std::isfinite(eps_c + e_corr)) return RTCC_EINVAL;
+    double* buf = nullptr;
+    const size_t cnt = (size_t)4 * nt + 2 * (size_t)nw;
+    if (cudaMalloc(&buf, cnt * 8) != cudaSuccess) { cudaGetLastError(); return RTCC_ENOMEM; }
+    double *dC = buf, *dG = buf + 2 * (size_t)nt, *dW = dG + 2 * (size_t)nt, *dA = dW + nw;
+    cudaMemcpy(dC, C, (size_t)2 * nt * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(dW, omega, (size_t)nw * 8, cudaMemcpyHostToDevice);
+    k_green<<<nblk(nt, 1024), 256>>>(nt, dt, dC, eps_c + e_corr, dG);
+    k_spectral<<<nw, RED_THREADS>>>(nt, dt, dG, eta, nw, dW, dA);
+    cudaError_t e = cudaMemcpy(A, dA, (size_t)nw * 8, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && G) e = cudaMemcpy(G, dG, (size_t)2 * nt * 8, cudaMemcpyDeviceToHost);
+    cudaFree(buf);
+    return e == cudaSuccess ? RTCC_OK : RTCC_ECUDA;
 }
 
 int rtcc_fp64_peak(double* tflops)

@@ -21,7 +21,7 @@ SYMBOLS = [
     "rtcc_create", "rtcc_destroy", "rtcc_sizes", "rtcc_residual", "rtcc_residual_energy", "rtcc_set_amplitudes",
     "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
-    "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror",
+    "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
 ]
 
 
@@ -59,6 +59,8 @@ def load():
         lib.rtcc_fp64_peak.argtypes = [P(d)]
         lib.rtcc_debug_buffer.argtypes = [vp, ctypes.c_char_p, vp, ll]; lib.rtcc_debug_buffer.restype = ll
         lib.rtcc_debug_gemm.argtypes = [i, i, i, vp, vp, vp, d, d, i]
+        lib.rtcc_build_fock.argtypes = [i, i, vp, vp, i, i, vp, ctypes.c_uint, vp]
+        lib.rtcc_spectral_function.argtypes = [i, d, vp, d, d, d, i, vp, vp, vp]
         lib.rtcc_last_cuda_error.argtypes = [vp]
         lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
         _lib = lib
@@ -105,6 +107,37 @@ def debug_gemm(A: np.ndarray, B: np.ndarray, C: np.ndarray | None = None, alpha=
     if rc:
         raise RtccError(rc, "rtcc_debug_gemm")
     return pc[0] + 1j * pc[1] if cplx else pc
+
+
+def build_fock(L, eps, core_spin: int, core_index: int):
+    """(N-1) Fock matrix f_pq = eps_p delta_pq - v_pc^qc from L[2,K,n,n] and eps[2,n]; numpy in, numpy out,
+    or torch CUDA tensors in, torch out."""
+    dev = _is_torch(L)
+    if dev:
+        import torch
+        K, n = L.shape[1], L.shape[2]
+        fock = torch.empty((2, n, n), dtype=torch.float64, device=L.device)
+        eps = eps.contiguous()
+    else:
+        L = np.ascontiguousarray(L, dtype=np.float64); eps = np.ascontiguousarray(eps, dtype=np.float64)
+        K, n = L.shape[1], L.shape[2]
+        fock = np.empty((2, n, n))
+    rc = load().rtcc_build_fock(n, K, _ptr(L), _ptr(eps), int(core_spin), int(core_index), _ptr(fock), 0 if dev else RTCC_HOST_PTRS, None)
+    if rc:
+        raise RtccError(rc, "rtcc_build_fock")
+    return fock
+
+
+def spectral_function(C, dt, eps_c, e_corr, eta, omega):
+    """G(tau_k) (complex array) and A(omega) from the recorded cumulant C(k dt) (Eqs. 3-4); host arrays."""
+    C = np.ascontiguousarray(C, dtype=np.complex128)
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    G = np.empty(C.size, dtype=np.complex128)
+    A = np.empty(omega.size)
+    rc = load().rtcc_spectral_function(C.size, float(dt), _ptr(C), float(eps_c), float(e_corr), float(eta), omega.size, _ptr(omega), _ptr(G), _ptr(A))
+    if rc:
+        raise RtccError(rc, "rtcc_spectral_function")
+    return G, A
 
 
 class Rtcc:

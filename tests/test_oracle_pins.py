@@ -390,3 +390,46 @@ def test_sampled_oracle_matches_full_oracle():
         # antisymmetry of the sampled values themselves
         i, j, a, b = so.so_of_packed_t2(0)
         assert abs(so.r2(j, i, a, b) + so.r2(i, j, a, b)) < 1e-13
+
+
+# ------------------------------------------------------------------ NEXT-3: (N-1) Fock matrix
+def test_fock_n1_is_eps_minus_antisymmetrised_core_integral():
+    """f_pq = eps_p delta_pq - <pc||qc>: the per-spin Coulomb/exchange formula must equal the spin-orbital definition
+    evaluated with the (independently pinned) antisymmetrised tensor of the C oracle, for the hole in either spin."""
+    oa, ob, va, vb, K = 2, 3, 4, 3, 6
+    L, fock_any = rand_problem(oa, ob, va, vb, K, 31)
+    prob = orc.Problem(oa, ob, va, vb, K, L, fock_any)
+    n = oa + va
+    rng = np.random.default_rng(3)
+    eps = rng.uniform(-2, 2, (2, n))
+    so = lambda s, p: (p if p < (ob if s else oa) else prob.d.no + (va if s else 0) + p - (ob if s else oa)) + (oa if s and p < ob else 0)
+    for cs, ci in ((0, oa), (1, 0), (0, 1)):
+        f = orc.build_fock_n1(L, eps, cs, ci)
+        c = so(cs, ci)
+        for s in range(2):
+            for p in range(n):
+                for q in range(n):
+                    ref = (eps[s, p] if p == q else 0.0) - prob.g[so(s, p), c, so(s, q), c]
+                    assert abs(f[s, p, q] - ref) < 1e-13
+        assert np.allclose(f, f.transpose(0, 2, 1))
+
+
+# ------------------------------------------------------------------ NEXT-2: Green's function / spectral function, Eqs. 3-4
+def test_spectral_function_closed_forms():
+    """C = 0: a single Lorentzian (eta/pi)/((w-e0)^2+eta^2) at e0 = eps_c + E_corr.  C = b (exp(-i W tau) - 1): the Poisson
+    satellite series exp(-b) sum_n b^n/n! Lorentzian(w - e0 - n W) (cumulant textbook result).  Long, finely sampled record."""
+    dt, nt, eta = 0.01, 40001, 0.05
+    tau = dt * np.arange(nt)
+    om = np.linspace(-3.0, 1.0, 81)
+    e0 = -1.3
+    lor = lambda x: (eta / np.pi) / (x * x + eta * eta)
+    G, A = orc.spectral_function(np.zeros(nt, complex), dt, -1.0, -0.3, eta, om)
+    assert np.abs(G[0] + 1j) < 1e-15 and np.allclose(np.abs(G), 1.0)
+    assert np.abs(A - lor(om - e0)).max() < 2e-4
+    b, W = 0.4, 0.7
+    C = b * (np.exp(-1j * W * tau) - 1.0)
+    _, A2 = orc.spectral_function(C, dt, -1.0, -0.3, eta, om)
+    from math import factorial
+    ref = sum(np.exp(-b) * b ** k / factorial(k) * lor(om - e0 - k * W) for k in range(25))
+    assert np.abs(A2 - ref).max() < 2e-4
+    assert abs(np.trapezoid(A2, om) - np.trapezoid(ref, om)) < 1e-3

@@ -246,3 +246,40 @@ def test_general_gemm_path_without_fused_small_kernels(rtcc, monkeypatch):
     monkeypatch.delenv("RTCC_NO_FUSED")
     monkeypatch.setenv("RTCC_NO_FUSED_FOCK", "1")
     check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+
+
+def test_build_fock_matches_oracle(rtcc):
+    """NEXT-3: (N-1) Fock matrix from L and eps, hole in either spin, host and device pointers."""
+    import torch
+    n, K = 23, 17
+    rng = np.random.default_rng(12)
+    L = rng.standard_normal((2, K, n, n)) * 0.3
+    L = 0.5 * (L + L.transpose(0, 1, 3, 2))
+    eps = rng.uniform(-20, 3, (2, n))
+    for cs, ci in ((0, 5), (1, 0), (1, n - 1)):
+        ref = orc.build_fock_n1(L, eps, cs, ci)
+        f = rtcc.build_fock(L, eps, cs, ci)
+        assert np.abs(f - ref).max() <= 1e-12 * np.abs(ref).max()
+        fd = rtcc.build_fock(torch.from_numpy(L).cuda(), torch.from_numpy(eps).cuda(), cs, ci)
+        assert np.array_equal(fd.cpu().numpy(), f)
+    with pytest.raises(rtcc.RtccError):
+        rtcc.build_fock(L, eps, 2, 0)
+
+
+def test_spectral_function_matches_oracle(rtcc):
+    """NEXT-2 (Eqs. 3-4): G(tau) and A(omega) from a recorded cumulant of a real propagation."""
+    cfg = inputs.CONFIGS["tiny"]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=0.2)
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)
+    ctx.set_solver(mode=1, tol=1e-10, max_micro=100)
+    Cs = [0j]
+    for _ in range(60):
+        ctx.step(cfg.dt)
+        Cs.append(ctx.cumulant()[0])
+    ctx.close()
+    Cs = np.array(Cs)
+    om = np.linspace(-25.0, -15.0, 101)
+    Go, Ao = orc.spectral_function(Cs, cfg.dt, -20.0, -0.25, 0.2, om)
+    G, A = rtcc.spectral_function(Cs, cfg.dt, -20.0, -0.25, 0.2, om)
+    assert np.abs(G - Go).max() <= 1e-12
+    assert np.abs(A - Ao).max() <= 1e-10 * np.abs(Ao).max()
