@@ -84,6 +84,18 @@ def run_reference(args, cfg):
     print(json.dumps(out))
 
 
+def aggregate_replicas(ms_local: float, steps: int, world: int, dist, device="cpu"):
+    """Replicas-only multi-GPU accounting: every rank runs the same workload on its own
+    GPU with no data-path collective; the job time is the MAX over ranks of the device-timed region and the whole-job value
+    is (ranks x steps) / that time.  Returns (ms_total, steps_per_s).  `dist` is torch.distributed or None."""
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if dist is not None and world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    return ms_total, world * steps / (ms_total * 1e-3)
+
+
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
@@ -169,12 +181,8 @@ def run_ours(args, cfg):
     launches, flops = ctx.counters()
     clocks = sampler.stop() if sampler else None
     ms = sum(a.elapsed_time(b) for a, b in evs)
-    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
+    ms_total, value = aggregate_replicas(ms, args.steps, world, dist, device="cuda")
     C, E = ctx.cumulant()
-    value = world * args.steps / (ms_total * 1e-3)
 
     # dominant kernel: the chained pp-ladder (3 launches per residual), timed live with CUDA events on the stream
     t1, t2 = inputs.random_amplitudes(cfg)
