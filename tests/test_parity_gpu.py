@@ -283,3 +283,39 @@ def test_spectral_function_matches_oracle(rtcc):
     G, A = rtcc.spectral_function(Cs, cfg.dt, -20.0, -0.25, 0.2, om)
     assert np.abs(G - Go).max() <= 1e-12
     assert np.abs(A - Ao).max() <= 1e-10 * np.abs(Ao).max()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("RTCC_RUN_MID"), reason="several minutes and ~12 GB of host memory: set RTCC_RUN_MID=1")
+def test_residual_mid_config_sampled(rtcc):
+    """BASELINE.json config 3 (Mid: o=24, v=200, n_chol=900) at full size: the general tcgemm path (no fused small kernels),
+    128x128 tiles at scale and the cluster ladder (clusters of 9 / 4 / 5) against the sampled-element oracle."""
+    import torch
+    from oracle.sampled import SampledOracle
+    cfg = inputs.CONFIGS["mid"]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=inputs.stabilised_sigma(cfg))
+    t1, t2 = inputs.random_amplitudes(cfg, std=2e-2)
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda())
+    r1d, r2d = ctx.residual(torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda())
+    r1, r2 = r1d.cpu().numpy(), r2d.cpu().numpy()
+    E = ctx.residual_energy()
+    ctx.close()
+    torch.cuda.empty_cache()
+    scale = max(np.abs(r1).max(), np.abs(r2).max())
+    so = SampledOracle(oa, ob, va, vb, K, L, fock, t1, t2)
+    d = so.d
+    naa = orc.npair(oa) * orc.npair(va)
+    nbb = orc.npair(ob) * orc.npair(vb)
+    rng = np.random.default_rng(4250)
+    picks = [0, naa - 1, naa, naa + nbb - 1, naa + nbb, d.n_t2 - 1]
+    picks += list(rng.integers(0, naa, 4)) + list(naa + rng.integers(0, nbb, 4)) + list(naa + nbb + rng.integers(0, d.n_t2 - naa - nbb, 8))
+    worst = 0.0
+    for k in picks:
+        i, j, a, b = so.so_of_packed_t2(int(k))
+        worst = max(worst, abs(so.r2(i, j, a, b) - r2[int(k)]))
+    for k in list(rng.integers(0, d.n_t1, 6)) + [0, d.n_t1 - 1]:
+        i, a = so.so_of_packed_t1(int(k))
+        worst = max(worst, abs(so.r1(i, a) - r1[int(k)]))
+    print("mid sampled parity: worst", worst, "scale", scale)
+    assert worst <= RTOL * scale, (worst, scale)
+    Eo = so.energy()
+    assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
