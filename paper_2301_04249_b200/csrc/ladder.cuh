@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
             const double* LAp = g.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA + (long long)kt0 * BLKA;
             const double* LBp = g.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB + (long long)kt0 * BLKB;
             int stage = 0; unsigned par = 1;
-            for (int ch = ch0; ch < ch1; ++ch) {
+            auto issue_g1 = [&](int ch) {
                 const int et = ch / nFt, ft = ch % nFt;
                 const double* curA = LAp + (long long)et * T1 * BLKA;
                 const double* curB = LBp + (long long)ft * T1 * BLKB;
@@ -337,7 +337,12 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
                     curA += BLKA; curB += BLKB;
                     if (++stage == LC_ST) { stage = 0; par ^= 1; }
                 }
+            };
+            if (ch0 < ch1) issue_g1(ch0);
+            for (int ch = ch0; ch < ch1; ++ch) {
+                if (ch + 1 < ch1) issue_g1(ch + 1);            // consumers build the next partial while this chunk is being gathered
                 if (has_col) {
+                    const int et = ch / nFt, ft = ch % nFt;
                     const double* curX = g.X + (((long long)(et * nFt + ft) * g.ncol + col) * T2) * BLKX;
                     for (int t = 0; t < T2; ++t) {
                         mbar_wait(&empty[stage], par);
@@ -365,7 +370,8 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
     const int u0 = (int)((long long)rank * UNITS / cl), u1 = (int)((long long)(rank + 1) * UNITS / cl);
 
     int stage = 0; unsigned par = 0, cpar = 0;
-    for (int ch = ch0; ch < ch1; ++ch) {
+    // GEMM-1 share of one chunk into acc1 (T1r tiles of the n_chol reduction)
+    auto gemm1 = [&]() {
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -391,7 +397,9 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
             if (lane == 0) mbar_arrive(&empty[stage]);
             if (++stage == LC_ST) { stage = 0; par ^= 1; }
         }
-        // partial W[(p,e),(q,f)] -> Ps[(p,q)][(e,f)]   (nobody reads Ps any more: barrier [1] of the previous chunk)
+    };
+    // partial W[(p,e),(q,f)] -> Ps[(p,q)][(e,f)], then tell the whole cluster (barrier [0])
+    auto publish = [&]() {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int m = w1m + 8 * i + lr;
@@ -404,10 +412,11 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
             }
         }
         __syncwarp();
-        if (lane == 0) {
-            asm volatile("fence.acq_rel.cluster;" ::: "memory");
-            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[0], r));
-        }
+        if (lane == 0)
+            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[0], r));      // release at cluster scope
+    };
+    if (ch0 < ch1) { gemm1(); publish(); }
+    for (int ch = ch0; ch < ch1; ++ch) {
         mbar_wait_cluster(&cbar[0], cpar);
         // reduce my slice over the cl partial tiles (fixed order) and hand the result to every CTA of the cluster
         for (int u = u0 + (tid & 255); u < u1; u += LD_NCONS) {
@@ -421,10 +430,11 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
             for (int r = 0; r < cl; ++r) st_cluster2(map_shared(Ws + off, r), s);
         }
         __syncwarp();
-        if (lane == 0) {
-            asm volatile("fence.acq_rel.cluster;" ::: "memory");
+        if (lane == 0)
             for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[1], r));
-        }
+        // software pipeline: the next chunk's GEMM-1 share runs while the other CTAs finish gathering this chunk
+        const bool more = ch + 1 < ch1;
+        if (more) gemm1();
         mbar_wait_cluster(&cbar[1], cpar);
         cpar ^= 1;
         if (has_col) {
@@ -450,6 +460,8 @@ __global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderC
                 if (++stage == LC_ST) { stage = 0; par ^= 1; }
             }
         }
+        // every CTA has finished reading Ps of this chunk (barrier [1]); my next partial may overwrite it now
+        if (more) publish();
     }
     if (has_col) {
         double* Yout = g.nsplit > 1 ? g.Ypart + (long long)split * g.nA * g.nB * g.ldY : g.Y;
