@@ -252,7 +252,7 @@ def run_ours(args, cfg):
             "config": {"workload": f"BASELINE.json configs[1] '{cfg.name}' (o={cfg.o}, v={cfg.v}, n_chol={cfg.K}, dt={cfg.dt}, "
                                    f"o_a/o_b/v_a/v_b={oa}/{ob}/{va}/{vb}), state from T=0",
                        "sigma": sigma, "sigma_note": "stabilised scale 0.2*sqrt(144/(v*d)); BASELINE.json's literal 0.3 diverges in step 2 (BASELINE.md section 4)",
-                       "solver": f"mode {BENCH_MODE} (plain Eq. 9 fixed point), tol {BENCH_TOL} (PAPER.md:139)",
+                       "solver": f"mode {BENCH_MODE} ({'plain Eq. 9 fixed point' if BENCH_MODE == 0 else 'denominator-preconditioned fixed point, NEXT-1'}), tol {BENCH_TOL} (PAPER.md:139)",
                        "micro_iters_per_step": micro / args.steps, "l2": "flushed between timed steps (252 MiB write)",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "workspace_bytes": ctx.workspace_bytes},
             "residual": {"ms": res_ms, "model_flops": f_model, "model_tflops": f_model / res_ms * 1e-9,
@@ -302,8 +302,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="small", choices=list(inputs.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", type=int, default=0, choices=[0, 1],
+                    help="0: the paper's plain fixed point of Eq. 9 (default, the headline); 1: denominator-preconditioned (NEXT-1)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    globals()["BENCH_MODE"] = args.mode
     cfg = inputs.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
