@@ -345,7 +345,9 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     if (g.Klo <= 0 || g.Klo >= g.K) g.Klo = 0x40000000;
     const int nbt = g.nb * g.nsb;
     const long long t128 = (long long)((g.M + 127) / 128) * ((g.N + 127) / 128) * nbt;
-    bool big = t128 >= (long long)(num_sms * 3) / 4 && g.M > 64 && g.N > 64;
+    // 128x128 tiles only when they fill the machine at least twice over; below that the 64x64 tiles (3 CTAs per SM, less
+    // padding) measured faster (Small: ring products of dimension 907)
+    bool big = t128 >= 2LL * num_sms && g.M > 64 && g.N > 64;
     {   // debugging override: RTCC_TILE=64 / 128 forces a tile configuration
         static int forced = -1;
         if (forced < 0) { const char* e = getenv("RTCC_TILE"); forced = e ? atoi(e) : 0; }
