@@ -186,7 +186,8 @@ def test_step_errors_leave_state_untouched(rtcc):
 
 def test_contraction_primitive_against_matmul(rtcc):
     rng = np.random.default_rng(0)
-    for (M, N, K) in [(5, 7, 3), (130, 70, 33), (300, 257, 1000), (20, 30, 5000), (129, 1, 77)]:
+    # the last shape is large enough (two full waves of 128x128 tiles) to run the big-tile kernel
+    for (M, N, K) in [(5, 7, 3), (130, 70, 33), (300, 257, 1000), (20, 30, 5000), (129, 1, 77), (2600, 2450, 70)]:
         A = rng.standard_normal((M, K)) + 1j * rng.standard_normal((M, K))
         B = rng.standard_normal((K, N)) + 1j * rng.standard_normal((K, N))
         C = rng.standard_normal((M, N)) + 1j * rng.standard_normal((M, N))
