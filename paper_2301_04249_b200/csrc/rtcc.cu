@@ -114,7 +114,9 @@ void ops_cc(TcGemm& g, const double* A, long long pA, const double* B, long long
 }
 void run(rtcc_ctx* c, TcGemm& g)
 {
-    if ((c->skipmask >> c->sec) & 1u) return;
+#ifdef RTCC_DEBUG_KNOBS
+    if ((c->skipmask >> c->sec) & 1u) return;      // timing experiments only (results are wrong when set)
+#endif
     const long long cap = c->ws_cap / 8;
     g.ws = c->ws + c->si * cap;
     int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops);
@@ -497,7 +499,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     BR(3);
     WAITEV(3, 0);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
-    if (!getenv("RTCC_SKIP_LADDER")) c->launches += ladder_launch(c->lb, ST, c->num_sms);   // (debug knob: timing of the other branches)
+    c->launches += ladder_launch(c->lb, ST, c->num_sms);
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], ST));
@@ -777,7 +779,9 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         for (int i = 0; i < 16; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
         for (int i = 0; i < 8; ++i) c->S[i] = c->st;
         c->si = 0;
+#ifdef RTCC_DEBUG_KNOBS
         if (const char* e = getenv("RTCC_SKIP_MASK")) c->skipmask = (unsigned)strtoul(e, nullptr, 0);
+#endif
         CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
 
         for (int s = 0; s < 2; ++s) {
