@@ -33,7 +33,7 @@ BENCH_MODE = 0
 BENCH_TOL = 1e-4
 BENCH_FIXED_MICRO = 0
 L2_BYTES = 126 * 2 ** 20
-LADDER_DRAM_BYTES_NCU = 92.7e6      # per launch, workload 'small' (profiles/r01c_topkernel_ncu.md: 65.2 MB read + 27.4 MB written)
+LADDER_DRAM_BYTES_NCU = 92.7e6      # per launch, workload 'small' (profiles/r01d_topkernel_ncu.md: 65.2 MB read + 27.4 MB written)
 
 
 def mac_model(o, v):
@@ -260,7 +260,7 @@ def run_ours(args, cfg):
             "roofline": {"bound": "tensor", "kernel": "ladder_kernel (one launch per residual: ab, aa, bb spin cases batched)",
                          "achieved": lad_model / lad_ms * 1e-9, "peak": peak, "unit": "TFLOP/s",
                          "frac": lad_model / lad_ms * 1e-9 / peak, "traffic": LADDER_DRAM_BYTES_NCU if cfg.name == "small" else None,
-                         "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r01c_topkernel_ncu.md)",
+                         "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r01d_topkernel_ncu.md)",
                          "ncu_dmma_pipe_active_pct": 92.6,
                          "executed_tflops": lad_exec / lad_ms * 1e-9, "ms": lad_ms, "algorithmic_flops": lad_model,
                          "peak_source": "measured live: register-resident FP64 DMMA loop (rtcc_fp64_peak); MEASURED_PEAKS.json has no fp64 figure"},
