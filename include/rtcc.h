@@ -57,6 +57,21 @@ int rtcc_create(rtcc_ctx** out, int o_alpha, int o_beta, int v_alpha, int v_beta
                 const double* L, const double* fock, unsigned flags, void* cuda_stream);
 void rtcc_destroy(rtcc_ctx* ctx);
 
+/* Process-wide tuning defaults read by rtcc_create (contexts already created are not affected; not thread-safe).  They
+ * select between code paths that compute the same result (the tests use them to force each path):
+ *   "fused" (1)             fused T1-dressing kernel when an n x n Cholesky slice fits in shared memory (0: GEMM path)
+ *   "fused_fock" (1)        fused dressed-Fock / F / singles kernels for small n (0: GEMM path)
+ *   "graph" (1)             replay one CUDA graph per residual evaluation (0: plain launches)
+ *   "stream_priorities" (1) latency-bound branches of the graph outrank the ladder branch
+ *   "gemm_tile" (0)         0: automatic, 64 or 128: force the contraction tile
+ *   "ladder_split" (0)      0: automatic, k >= 1: force k slices of the (e,f) plane per ladder work item
+ *   "max_cluster" (16)      largest thread-block cluster the wide ladder kernel may use (1..16)
+ *   "ladder_cluster" (0)    0: automatic, k >= 1: force clusters of k CTAs in the wide ladder kernel
+ *   "ladder_tiles" (5)      column tiles one CTA of the wide ladder kernel may hold (1..5; 4 of them parked in tensor memory)
+ *   "reset"                 back to the defaults (value ignored)
+ * Returns RTCC_EINVAL for an unknown name or a value out of range. */
+int rtcc_set_default_option(const char* name, int value);
+
 /* n_t1, n_t2: complex element counts of the packed arrays; workspace_bytes: device memory held. */
 int rtcc_sizes(const rtcc_ctx* ctx, long long* n_t1, long long* n_t2, long long* workspace_bytes);
 
@@ -91,6 +106,11 @@ int rtcc_reset_counters(rtcc_ctx* ctx);
 int rtcc_set_timing(rtcc_ctx* ctx, int on);
 int rtcc_ladder_timing(const rtcc_ctx* ctx, double* ms, double* flops, double* model_flops);
 
+/* Launch plan of the pp-ladder for spin case 0, 1, 2 (those with a non-empty block, in the order ab, aa, bb; RTCC_EINVAL past
+ * the last): out = { stacked Re|Im columns, column tile width, column tiles, CTAs per cluster (0: narrow batched kernel),
+ * column groups, (e,f) slices, row tiles, SMs the clusters can occupy }. */
+int rtcc_ladder_plan(const rtcc_ctx* ctx, int spin_case, int out[8]);
+
 /* (N-1)-electron Fock matrix from the Cholesky vectors and the orbital energies of the N-electron reference
  * (f_pq = eps_p delta_pq - v_pc^qc, c = core-hole spin-orbital; v_pq^rs = <pq||rs>):
  *   fock[s][p][q] = eps[s][p] delta_pq - sum_Q L[s][Q][p][q] L[cs][Q][c][c] + delta(s,cs) sum_Q L[s][Q][p][c] L[s][Q][c][q]
@@ -118,6 +138,7 @@ long long rtcc_debug_buffer(const rtcc_ctx* ctx, const char* name, double* out, 
  * HOST arrays; cplx != 0 treats A, B, C as planar complex ([2][rows][cols]). */
 int rtcc_debug_gemm(int M, int N, int K, const double* A, const double* B, double* C, double alpha, double beta, int cplx);
 
+/* cudaError_t behind the most recent RTCC_ECUDA / RTCC_ENOMEM of this context; ctx == NULL: of the most recent failed rtcc_create. */
 int rtcc_last_cuda_error(const rtcc_ctx* ctx);
 const char* rtcc_strerror(int code);
 

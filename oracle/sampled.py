@@ -8,15 +8,70 @@ index slices this element touches".  It shares no code with the CUDA path and do
 
 Pinned by tests/test_oracle_pins.py::test_sampled_oracle_matches_full_oracle (agreement with the determinant-pinned
 tier-A oracle to 1e-13 on complex amplitudes with a general Fock matrix).
+
+``SampledOracleC`` (rtcc_sampled.c) evaluates the same elements with plain C loops straight off the packed blocks; it is
+the one that fits BASELINE.json configs 3-5.  Pinned the same way (test_sampled_c_oracle_matches_full_oracle).
 """
 from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
 
 import numpy as np
 
 from . import oracle as orc
 
 
-class SampledOracle:
+class _PackedIndex:
+    """Packed t2 / t1 position -> spin-orbital indices (shared by both sampled oracles; needs self.d)."""
+
+    def so_of_packed_t2(self, k):
+        d = self.d
+        nss = [orc.npair(d.oa) * orc.npair(d.va), orc.npair(d.ob) * orc.npair(d.vb)]
+        off_o, off_v = [0, d.oa], [0, d.va]
+        for s, (o, v) in enumerate(((d.oa, d.va), (d.ob, d.vb))):
+            if k < nss[s]:
+                pij, pab = divmod(k, orc.npair(v))
+                j = int((1 + np.sqrt(1 + 8 * pij)) // 2)
+                while orc.pair(0, j) > pij:
+                    j -= 1
+                while orc.pair(0, j + 1) <= pij:
+                    j += 1
+                i = pij - orc.pair(0, j)
+                b = int((1 + np.sqrt(1 + 8 * pab)) // 2)
+                while orc.pair(0, b) > pab:
+                    b -= 1
+                while orc.pair(0, b + 1) <= pab:
+                    b += 1
+                a = pab - orc.pair(0, b)
+                return off_o[s] + i, off_o[s] + j, off_v[s] + a, off_v[s] + b
+            k -= nss[s]
+        B = k % d.vb; k //= d.vb
+        a = k % d.va; k //= d.va
+        J = k % d.ob; i = k // d.ob
+        return i, d.oa + J, a, d.va + B
+
+    def so_of_packed_t1(self, k):
+        d = self.d
+        if k < d.oa * d.va:
+            return divmod(k, d.va)
+        i, a = divmod(k - d.oa * d.va, d.vb)
+        return d.oa + i, d.va + a
+
+    def packed_of_so_t2(self, i, j, a, b):
+        """Inverse of so_of_packed_t2 for a canonical element (same spin: i<j, a<b; mixed: i alpha, j beta, a alpha, b beta)."""
+        d = self.d
+        naa = orc.npair(d.oa) * orc.npair(d.va)
+        nbb = orc.npair(d.ob) * orc.npair(d.vb)
+        if j < d.oa:
+            return orc.pair(i, j) * orc.npair(d.va) + orc.pair(a, b)
+        if i >= d.oa:
+            return naa + orc.pair(i - d.oa, j - d.oa) * orc.npair(d.vb) + orc.pair(a - d.va, b - d.va)
+        return naa + nbb + ((i * d.ob + (j - d.oa)) * d.va + a) * d.vb + (b - d.va)
+
+
+class SampledOracle(_PackedIndex):
     def __init__(self, oa, ob, va, vb, K, L, fock, t1p, t2p):
         self.d = d = orc.Dims(oa, ob, va, vb, K)
         n = oa + va
@@ -128,36 +183,90 @@ class SampledOracle:
         return complex(np.sum(f[:no, no:] * self.t1) + 0.25 * np.sum(self.oovv * self.t2)
                        + 0.5 * np.einsum("ijab,ia,jb->", self.oovv, self.t1, self.t1))
 
-    # ---- packed-index helpers for the tests: map a packed t2 / t1 position to spin-orbital indices
-    def so_of_packed_t2(self, k):
-        d = self.d
-        nss = [orc.npair(d.oa) * orc.npair(d.va), orc.npair(d.ob) * orc.npair(d.vb)]
-        off_o, off_v = [0, d.oa], [0, d.va]
-        for s, (o, v) in enumerate(((d.oa, d.va), (d.ob, d.vb))):
-            if k < nss[s]:
-                pij, pab = divmod(k, orc.npair(v))
-                j = int((1 + np.sqrt(1 + 8 * pij)) // 2)
-                while orc.pair(0, j) > pij:
-                    j -= 1
-                while orc.pair(0, j + 1) <= pij:
-                    j += 1
-                i = pij - orc.pair(0, j)
-                b = int((1 + np.sqrt(1 + 8 * pab)) // 2)
-                while orc.pair(0, b) > pab:
-                    b -= 1
-                while orc.pair(0, b + 1) <= pab:
-                    b += 1
-                a = pab - orc.pair(0, b)
-                return off_o[s] + i, off_o[s] + j, off_v[s] + a, off_v[s] + b
-            k -= nss[s]
-        B = k % d.vb; k //= d.vb
-        a = k % d.va; k //= d.va
-        J = k % d.ob; i = k // d.ob
-        return i, d.oa + J, a, d.va + B
 
-    def so_of_packed_t1(self, k):
-        d = self.d
-        if k < d.oa * d.va:
-            return divmod(k, d.va)
-        i, a = divmod(k - d.oa * d.va, d.vb)
-        return d.oa + i, d.va + a
+# ----------------------------------------------------------------------------------------------------------------------
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "rtcc_sampled.c")
+_CLIB = os.path.join(_HERE, "librtcc_sampled.so")
+_clib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile rtcc_sampled.c with gcc (-O2, OpenMP).  Returns the .so path."""
+    if force or not os.path.exists(_CLIB) or os.path.getmtime(_CLIB) < os.path.getmtime(_CSRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _CLIB, _CSRC, "-lm"])
+    return _CLIB
+
+
+def _cload():
+    global _clib
+    if _clib is None:
+        build()
+        lib = ctypes.CDLL(_CLIB)
+        dp, i, vp = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_void_p
+        lib.sorc_num_threads.restype = i
+        lib.sorc_create.argtypes = [i, i, i, i, i, dp, dp, dp, dp]
+        lib.sorc_create.restype = vp
+        lib.sorc_destroy.argtypes = [vp]
+        lib.sorc_destroy.restype = None
+        lib.sorc_drop_slices.argtypes = [vp]
+        lib.sorc_drop_slices.restype = None
+        lib.sorc_r2.argtypes = [vp, i, i, i, i, dp]
+        lib.sorc_r2.restype = i
+        lib.sorc_r1.argtypes = [vp, i, i, dp]
+        lib.sorc_r1.restype = i
+        lib.sorc_energy.argtypes = [vp, dp]
+        lib.sorc_energy.restype = None
+        _clib = lib
+    return _clib
+
+
+class SampledOracleC(_PackedIndex):
+    """Same elements as ``SampledOracle`` from rtcc_sampled.c: plain C loops straight off the packed blocks and the per-spin
+    Cholesky vectors, so that BASELINE.json configs 3-5 (where the numpy version's spin-orbital copies of t2 do not fit in
+    host memory) can be checked.  Pinned to the full oracle in tests/test_oracle_pins.py."""
+
+    def __init__(self, oa, ob, va, vb, K, L, fock, t1p, t2p):
+        self.d = orc.Dims(oa, ob, va, vb, K)
+        n = oa + va
+        L = np.ascontiguousarray(L, dtype=np.float64).reshape(2, K, n, n)
+        fock = np.ascontiguousarray(fock, dtype=np.float64).reshape(2, n, n)
+        t1p = np.ascontiguousarray(t1p, dtype=np.complex128)
+        t2p = np.ascontiguousarray(t2p, dtype=np.complex128)
+        assert t1p.size == self.d.n_t1 and t2p.size == self.d.n_t2
+        dp = ctypes.POINTER(ctypes.c_double)
+        self._lib = _cload()
+        self._h = self._lib.sorc_create(oa, ob, va, vb, K, L.ctypes.data_as(dp), fock.ctypes.data_as(dp),
+                                        t1p.ctypes.data_as(dp), t2p.ctypes.data_as(dp))
+        if not self._h:
+            raise MemoryError("sampled oracle: allocation failed")
+        self._out = np.zeros(2)
+        self._dp = self._out.ctypes.data_as(dp)
+
+    def close(self):
+        if self._h:
+            self._lib.sorc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def drop_slices(self):
+        self._lib.sorc_drop_slices(self._h)
+
+    def r2(self, i, j, a, b):
+        if self._lib.sorc_r2(self._h, int(i), int(j), int(a), int(b), self._dp):
+            raise MemoryError("sampled oracle: allocation failed")
+        return complex(self._out[0], self._out[1])
+
+    def r1(self, i, a):
+        if self._lib.sorc_r1(self._h, int(i), int(a), self._dp):
+            raise MemoryError("sampled oracle: allocation failed")
+        return complex(self._out[0], self._out[1])
+
+    def energy(self):
+        self._lib.sorc_energy(self._h, self._dp)
+        return complex(self._out[0], self._out[1])

@@ -39,8 +39,8 @@ struct LadderCase {
     int nsplit;                           // slices of the (e,f) chunk list
     int nt2;                              // column tile width: 64 or 128
     int ncol;                             // column tiles
-    int cl;                               // CTAs per cluster sharing one W chunk (1: plain kernel); ncol > 1 only
-    int ngrp;                             // column-tile groups of cl tiles each
+    int cl;                               // 0: batched narrow kernel (one column tile); >= 1: wide kernel, CTAs per cluster
+    int ngrp;                             // wide kernel: column-tile groups (each group rebuilds the W chunks)
     int item0;                            // first work item of this case
 };
 struct LadderBatch {
@@ -250,13 +250,29 @@ __global__ void __launch_bounds__(LD_NTH) ladder_kernel(const LadderBatch b)
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Wide amplitudes (more than one column tile): a thread-block CLUSTER of cl CTAs owns one (p,q) row tile.  CTA r
-// keeps the accumulators of column tile r.  Each W chunk is built ONCE per cluster: the n_chol reduction of GEMM-1 is
-// split across the CTAs, the partial tiles are summed through distributed shared memory in a fixed order
-// (reduce-scatter + all-gather, deterministic) and every CTA then applies the complete chunk to its own columns.
-constexpr int LC_ST = 3;
-constexpr size_t ladder_cluster_smem()
-{ return sizeof(double) * (LC_ST * (size_t)LD_STAGE + 2 * (size_t)LD_R * LD_LDW) + (2 * LC_ST + 2) * sizeof(unsigned long long); }
+// Wide amplitudes (more than one 128-column tile).  One CTA keeps the accumulators of up to LW_MAXC column tiles of its
+// 64-row tile: the live tile in registers (FP64 DMMA accumulates in registers only), the others parked in TENSOR MEMORY
+// (tcgen05.alloc / tcgen05.ld / tcgen05.st: 8 warps x 32 lanes x 256 columns = 4 parked tiles) and swapped in place when the
+// CTA moves to the next tile; tiles are visited in alternating order so that a chunk ends on the tile the next one starts on.
+// A thread-block CLUSTER of cl CTAs covers cl * LW_MAXC column tiles.  Every W chunk is built ONCE per cluster: CTA r builds
+// the chunks g = r (mod cl) completely (all of n_chol, one cl-th of it per step so that every CTA does the same work in every
+// step), writes the finished chunk into one of two shared-memory slots and sends it to the same slot of every other CTA with
+// one bulk async copy through distributed shared memory (cp.async.bulk shared::cta -> shared::cluster, completion on the
+// receiver's mbarrier) -- the consumer warps never touch remote memory.  Slot reuse is guarded by "credit" mbarriers at the
+// builder that every consumer warp of the cluster arrives on when it has finished a chunk.  Fixed summation order
+// throughout: bit-reproducible.
+constexpr int LW_ST = 3;
+constexpr int LW_MAXC = 5;
+constexpr int LW_NTH = 384;                             // two consumer warpgroups + one producer warpgroup (register reallocation)
+constexpr int LW_WSLOT = LD_R * LD_LDW;                 // doubles per W slot
+constexpr int LW_NBAR = 2 * LW_ST + 4;                  // full[ST], empty[ST], wfull[2], credit[2]
+constexpr size_t ladder_wide_smem()
+{ return sizeof(double) * (LW_ST * (size_t)LD_STAGE + 2 * (size_t)LW_WSLOT) + LW_NBAR * sizeof(unsigned long long) + 16; }
+
+struct LadderWide {
+    LadderCase c[3];        // cases batched in one launch share the cluster size
+    int ncase, NQ, cl;
+};
 
 __device__ __forceinline__ unsigned cluster_rank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ unsigned map_shared(const void* p, unsigned rank)
@@ -265,10 +281,6 @@ __device__ __forceinline__ unsigned map_shared(const void* p, unsigned rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
     return r;
 }
-__device__ __forceinline__ double2 ld_cluster2(unsigned addr)
-{ double2 v; asm volatile("ld.shared::cluster.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory"); return v; }
-__device__ __forceinline__ void st_cluster2(unsigned addr, double2 v)
-{ asm volatile("st.shared::cluster.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory"); }
 __device__ __forceinline__ void mbar_arrive_cluster(unsigned remote_addr)
 { asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote_addr) : "memory"); }
 __device__ __forceinline__ void mbar_wait_cluster(unsigned long long* b, unsigned parity)
@@ -280,209 +292,308 @@ __device__ __forceinline__ void mbar_wait_cluster(unsigned long long* b, unsigne
                      : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
     } while (!ok);
 }
+// bulk async copy from this CTA's shared memory into a peer's (addresses of the peer obtained with mapa)
+__device__ __forceinline__ void bulk_s2peer(unsigned dst_cluster_addr, const void* src, unsigned bytes, unsigned bar_cluster_addr)
+{
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster_addr), "r"((unsigned)__cvta_generic_to_shared(src)), "r"(bytes), "r"(bar_cluster_addr) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{ asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
-__global__ void __launch_bounds__(LD_NTH, 1) ladder_cluster_kernel(const LadderCase g, const int NQ)
+// ---- tensor memory: 8 consecutive 32-bit columns of this thread's lane <-> 4 doubles
+__device__ __forceinline__ void tmem_ld8(unsigned taddr, unsigned (&r)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(unsigned taddr, double d0, double d1, double d2, double d3)
+{
+    asm volatile("{\n .reg .b32 l0, h0, l1, h1, l2, h2, l3, h3;\n"
+                 " mov.b64 {l0, h0}, %1;\n mov.b64 {l1, h1}, %2;\n mov.b64 {l2, h2}, %3;\n mov.b64 {l3, h3}, %4;\n"
+                 " tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {l0, h0, l1, h1, l2, h2, l3, h3};\n}"
+                 ::"r"(taddr), "d"(d0), "d"(d1), "d"(d2), "d"(d3) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// swap the 32 accumulators of this thread with the parked tile at taddr (64 columns), 4 doubles at a time
+__device__ __forceinline__ void tmem_exchange(unsigned taddr, double (&acc)[4][4][2])
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            unsigned in[8];
+            const unsigned a = taddr + 16 * i + 8 * h;
+            tmem_ld8(a, in);
+            tmem_wait_ld();
+            tmem_st8(a, acc[i][2 * h][0], acc[i][2 * h][1], acc[i][2 * h + 1][0], acc[i][2 * h + 1][1]);
+            acc[i][2 * h][0] = __hiloint2double((int)in[1], (int)in[0]);
+            acc[i][2 * h][1] = __hiloint2double((int)in[3], (int)in[2]);
+            acc[i][2 * h + 1][0] = __hiloint2double((int)in[5], (int)in[4]);
+            acc[i][2 * h + 1][1] = __hiloint2double((int)in[7], (int)in[6]);
+        }
+    tmem_wait_st();
+}
+__device__ __forceinline__ void tmem_zero64(unsigned taddr)
+{
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tmem_st8(taddr + 8 * i, 0.0, 0.0, 0.0, 0.0);
+    tmem_wait_st();
+}
+
+__global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide b)
 {
     constexpr int NT2 = 128, LDX2 = NT2 + 4, T2 = LD_K2 / LD_BK;
+    constexpr int BLKA = LD_BK * LD_LDA1, BLKB = LD_BK * LD_LDB1, BLKX = LD_BK * LDX2;
     extern __shared__ __align__(128) double smem[];
     double* stg = smem;
-    double* Ws = smem + LC_ST * LD_STAGE;
-    double* Ps = Ws + LD_R * LD_LDW;
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(Ps + LD_R * LD_LDW);
-    unsigned long long* empty = full + LC_ST;
-    unsigned long long* cbar = empty + LC_ST;          // [0]: partial tiles written, [1]: reduced chunk distributed
+    double* Wsl = smem + LW_ST * LD_STAGE;                                   // two W slots
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(Wsl + 2 * LW_WSLOT);
+    unsigned long long* empty = full + LW_ST;
+    unsigned long long* wfull = empty + LW_ST;                                // [2]: chunk landed in slot
+    unsigned long long* credit = wfull + 2;                                   // [2]: slot released by every consumer warp of the cluster
+    unsigned* tmem_base_p = reinterpret_cast<unsigned*>(credit + 2);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int cl = g.cl;
+    const int cl = b.cl, NQ = b.NQ;
     const int rank = (int)cluster_rank();
     int item = blockIdx.x / cl;
+    int ci = 0;
+    if (b.ncase > 1 && item >= b.c[1].item0) ci = 1;
+    if (b.ncase > 2 && item >= b.c[2].item0) ci = 2;
+    const LadderCase& g = b.c[ci];
+    item -= g.item0;
     const int split = item % g.nsplit; item /= g.nsplit;
     const int grp = item % g.ngrp;
     const int2 tl = g.tiles[item / g.ngrp];
     const int p0 = tl.x, q0 = tl.y;
-    const int col = grp * cl + rank;
-    const bool has_col = col < g.ncol;
-    const int x0 = col * NT2;
+    // column tiles of this CTA: group grp holds tiles [gt0, gt1), split evenly over the cl ranks
+    const int gt0 = (int)((long long)grp * g.ncol / g.ngrp), gt1 = (int)((long long)(grp + 1) * g.ncol / g.ngrp);
+    const int ct0 = gt0 + (int)((long long)rank * (gt1 - gt0) / cl), ct1 = gt0 + (int)((long long)(rank + 1) * (gt1 - gt0) / cl);
+    const int Ct = ct1 - ct0;                                                 // 0 .. LW_MAXC
     const int nEt = (g.vA + LD_PE - 1) / LD_PE, nFt = (g.vB + LD_PF - 1) / LD_PF;
     const int nchunk = nEt * nFt;
     const int ch0 = (int)((long long)split * nchunk / g.nsplit), ch1 = (int)((long long)(split + 1) * nchunk / g.nsplit);
+    const int G = ch1 - ch0;
     const int T1 = NQ / LD_BK;
-    const int kt0 = (int)((long long)rank * T1 / cl), kt1 = (int)((long long)(rank + 1) * T1 / cl);   // my share of the n_chol reduction
-    const int T1r = kt1 - kt0;
 
     if (tid == 0) {
-        for (int s = 0; s < LC_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
-        mbar_init(&cbar[0], 8 * cl); mbar_init(&cbar[1], 8 * cl);
+        for (int s = 0; s < LW_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&wfull[s], 1); mbar_init(&credit[s], 8 * cl); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // chunks 0 and 1 arrive from their builders without a preceding release of the slot: arm their barriers here
+        for (int s = 0; s < 2; ++s)
+            if (s < G && s % cl != rank) mbar_expect_tx(&wfull[s], LW_WSLOT * 8);
     }
-    __syncthreads();
-    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");   // every CTA's barriers exist
-
     if (warp == 8) {
-        if (lane == 0) {
-            constexpr int BLKA = LD_BK * LD_LDA1, BLKB = LD_BK * LD_LDB1, BLKX = LD_BK * LDX2;
-            const double* LAp = g.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA + (long long)kt0 * BLKA;
-            const double* LBp = g.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB + (long long)kt0 * BLKB;
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((unsigned)__cvta_generic_to_shared(tmem_base_p)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const unsigned tmem_base = *tmem_base_p;
+    cluster_sync_all();                                                       // every CTA's barriers exist
+
+    // Both roles walk the same schedule.  Chunk g (0-based within [ch0, ch1)) is built by rank g % cl, published at the start
+    // of step g-1 and consumed in step g.  A build is spread over the cl steps before its publication.
+    if (warp >= 8) {
+        // producer warpgroup: hands its registers to the consumers (the kernel is compiled for 168 registers per thread,
+        // 3 warpgroups; the consumers need ~220 to keep both accumulator sets out of local memory)
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
+        if (warp == 8 && lane == 0) {
+            const double* LAp = g.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA;
+            const double* LBp = g.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB;
             int stage = 0; unsigned par = 1;
-            auto issue_g1 = [&](int ch) {
+            auto issue_L = [&](int ch, int k0, int k1) {
                 const int et = ch / nFt, ft = ch % nFt;
-                const double* curA = LAp + (long long)et * T1 * BLKA;
-                const double* curB = LBp + (long long)ft * T1 * BLKB;
-                for (int t = 0; t < T1r; ++t) {
+                const double* curA = LAp + ((long long)et * T1 + k0) * BLKA;
+                const double* curB = LBp + ((long long)ft * T1 + k0) * BLKB;
+                for (int t = k0; t < k1; ++t) {
                     mbar_wait(&empty[stage], par);
                     double* sb = stg + stage * LD_STAGE;
                     mbar_expect_tx(&full[stage], (BLKA + BLKB) * 8);
                     bulk_g2s(sb, curA, BLKA * 8, &full[stage]);
                     bulk_g2s(sb + BLKA, curB, BLKB * 8, &full[stage]);
                     curA += BLKA; curB += BLKB;
-                    if (++stage == LC_ST) { stage = 0; par ^= 1; }
+                    if (++stage == LW_ST) { stage = 0; par ^= 1; }
                 }
             };
-            if (ch0 < ch1) issue_g1(ch0);
-            for (int ch = ch0; ch < ch1; ++ch) {
-                if (ch + 1 < ch1) issue_g1(ch + 1);            // consumers build the next partial while this chunk is being gathered
-                if (has_col) {
+            int gb = rank, kdone = 0;
+            for (int s = -2; s < G; ++s) {
+                if (s >= -1 && s + 1 < G && (s + 1) % cl == rank) { gb = s + 1 + cl; kdone = 0; }
+                if (gb < G && kdone < T1) {
+                    const int rem = gb - 1 - s;
+                    const int nk = (T1 - kdone + rem - 1) / rem;
+                    issue_L(ch0 + gb, kdone, kdone + nk);
+                    kdone += nk;
+                }
+                if (s >= 0 && Ct > 0) {
+                    const int ch = ch0 + s;
                     const int et = ch / nFt, ft = ch % nFt;
-                    const double* curX = g.X + (((long long)(et * nFt + ft) * g.ncol + col) * T2) * BLKX;
-                    for (int t = 0; t < T2; ++t) {
-                        mbar_wait(&empty[stage], par);
-                        mbar_expect_tx(&full[stage], BLKX * 8);
-                        bulk_g2s(stg + stage * LD_STAGE, curX, BLKX * 8, &full[stage]);
-                        curX += BLKX;
-                        if (++stage == LC_ST) { stage = 0; par ^= 1; }
+                    const double* Xc = g.X + ((long long)(et * nFt + ft) * g.ncol) * T2 * BLKX;
+                    for (int u = 0; u < Ct; ++u) {
+                        const int tile = (s & 1) ? Ct - 1 - u : u;
+                        const double* curX = Xc + (long long)(ct0 + tile) * T2 * BLKX;
+                        for (int t = 0; t < T2; ++t) {
+                            mbar_wait(&empty[stage], par);
+                            mbar_expect_tx(&full[stage], BLKX * 8);
+                            bulk_g2s(stg + stage * LD_STAGE, curX, BLKX * 8, &full[stage]);
+                            curX += BLKX;
+                            if (++stage == LW_ST) { stage = 0; par ^= 1; }
+                        }
                     }
                 }
             }
         }
+        __syncwarp();
     } else {
-    // ---------------- consumers
-    const int lr = lane >> 2, lc = lane & 3;
-    double acc2[4][4][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
-    double acc1[4][4][2];
-    const int w1m = (warp >> 1) * 32, w1n = (warp & 1) * 32;
-    const int w2m = (warp >> 2) * 32, w2n = (warp & 3) * 32;
-    // my slice of the 64 x 128 chunk in double2 units (reduce-scatter)
-    constexpr int UNITS = LD_R * LD_K2 / 2;
-    const int u0 = (int)((long long)rank * UNITS / cl), u1 = (int)((long long)(rank + 1) * UNITS / cl);
-
-    int stage = 0; unsigned par = 0, cpar = 0;
-    // GEMM-1 share of one chunk into acc1 (T1r tiles of the n_chol reduction)
-    auto gemm1 = [&]() {
+        // ---------------- consumers
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
+        const int lr = lane >> 2, lc = lane & 3;
+        double acc2[4][4][2], acc1[4][4][2];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
-        for (int t = 0; t < T1r; ++t) {
-            mbar_wait(&full[stage], par);
-            const double* sb = stg + stage * LD_STAGE;
-            const double* as = sb + lc * LD_LDA1 + w1m + lr;
-            const double* bs = sb + LD_BK * LD_LDA1 + lc * LD_LDB1 + w1n + lr;
+            for (int j = 0; j < 4; ++j) acc2[i][j][0] = acc2[i][j][1] = acc1[i][j][0] = acc1[i][j][1] = 0.0;
+        const int w1m = (warp >> 1) * 32, w1n = (warp & 1) * 32;
+        const int w2m = (warp >> 2) * 32, w2n = (warp & 3) * 32;
+        // this warp's tensor-memory region: lanes 32 (warp % 4) .., columns 256 (warp / 4) + 64 slot
+        const unsigned tm0 = tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
+        for (int s = 0; s + 1 < Ct; ++s) tmem_zero64(tm0 + 64 * s);      // parked tiles start at zero
+
+        int stage = 0; unsigned par = 0;
+        unsigned cpar = 0u;                                                   // bit sl: parity of credit[sl]
+        // acc1 = W[(p,e),(q,f)] of chunk gc -> slot gc % 2 as [(p,q)][(e,f)], here and in every other CTA of the cluster
+        auto publish = [&](int gc) {
+            const int sl = gc & 1;
+            if (gc >= 2) { mbar_wait_cluster(&credit[sl], (cpar >> sl) & 1u); cpar ^= 1u << sl; }     // every warp of the cluster is done with chunk gc-2
+            double* Ws = Wsl + sl * LW_WSLOT;
 #pragma unroll
-            for (int ks = 0; ks < LD_BK / 4; ++ks) {
-                double a[4], b[4];
+            for (int i = 0; i < 4; ++i) {
+                const int m = w1m + 8 * i + lr;
+                const int p = m / LD_PE, e = m % LD_PE;
 #pragma unroll
-                for (int i = 0; i < 4; ++i) a[i] = as[ks * 4 * LD_LDA1 + 8 * i];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) b[j] = bs[ks * 4 * LD_LDB1 + 8 * j];
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], a[i], b[j]);
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[stage]);
-            if (++stage == LC_ST) { stage = 0; par ^= 1; }
-        }
-    };
-    // partial W[(p,e),(q,f)] -> Ps[(p,q)][(e,f)], then tell the whole cluster (barrier [0])
-    auto publish = [&]() {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int m = w1m + 8 * i + lr;
-            const int p = m / LD_PE, e = m % LD_PE;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int n = w1n + 8 * j + 2 * lc;
-                const int q = n / LD_PF, f = n % LD_PF;
-                *reinterpret_cast<double2*>(&Ps[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]) = make_double2(acc1[i][j][0], acc1[i][j][1]);
-            }
-        }
-        __syncwarp();
-        if (lane == 0)
-            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[0], r));      // release at cluster scope
-    };
-    if (ch0 < ch1) { gemm1(); publish(); }
-    for (int ch = ch0; ch < ch1; ++ch) {
-        mbar_wait_cluster(&cbar[0], cpar);
-        // reduce my slice over the cl partial tiles (fixed order) and hand the result to every CTA of the cluster
-        for (int u = u0 + (tid & 255); u < u1; u += LD_NCONS) {
-            const int row = u / (LD_K2 / 2), c2 = u % (LD_K2 / 2);
-            const int off = row * LD_LDW + 2 * c2;
-            double2 s = make_double2(0.0, 0.0);
-            for (int r = 0; r < cl; ++r) {
-                double2 v = ld_cluster2(map_shared(Ps + off, r));
-                s.x += v.x; s.y += v.y;
-            }
-            for (int r = 0; r < cl; ++r) st_cluster2(map_shared(Ws + off, r), s);
-        }
-        __syncwarp();
-        if (lane == 0)
-            for (int r = 0; r < cl; ++r) mbar_arrive_cluster(map_shared(&cbar[1], r));
-        // software pipeline: the next chunk's GEMM-1 share runs while the other CTAs finish gathering this chunk
-        const bool more = ch + 1 < ch1;
-        if (more) gemm1();
-        mbar_wait_cluster(&cbar[1], cpar);
-        cpar ^= 1;
-        if (has_col) {
-            for (int t = 0; t < T2; ++t) {
-                mbar_wait(&full[stage], par);
-                const double* sb = stg + stage * LD_STAGE;
-                const double* ws = Ws + (w2m + lr) * LD_LDW + t * LD_BK + lc;
-                const double* xs = sb + lc * LDX2 + w2n + lr;
-#pragma unroll
-                for (int ks = 0; ks < LD_BK / 4; ++ks) {
-                    double a[4], b[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) a[i] = ws[8 * i * LD_LDW + ks * 4];
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) b[j] = xs[ks * 4 * LDX2 + 8 * j];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], a[i], b[j]);
+                for (int j = 0; j < 4; ++j) {
+                    const int n = w1n + 8 * j + 2 * lc;
+                    const int q = n / LD_PF, f = n % LD_PF;
+                    *reinterpret_cast<double2*>(&Ws[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]) = make_double2(acc1[i][j][0], acc1[i][j][1]);
+                    acc1[i][j][0] = acc1[i][j][1] = 0.0;
                 }
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes -> visible to the bulk copies
+            bar_consumers();
+            if (tid == 0) {
+                for (int r = 1; r < cl; ++r) {
+                    const unsigned peer = (unsigned)((rank + r) % cl);
+                    bulk_s2peer(map_shared(Ws, peer), Ws, LW_WSLOT * 8, map_shared(&wfull[sl], peer));
+                }
+                mbar_arrive(&wfull[sl]);
+            }
+        };
+
+        // steps -2 and -1 are the prologue: the first chunk of rank r is built over the steps -2 .. r-2
+        int gb = rank, kdone = 0;
+        for (int s = -2; s < G; ++s) {
+            if (s >= -1 && s + 1 < G && (s + 1) % cl == rank) { publish(s + 1); gb = s + 1 + cl; kdone = 0; }
+            if (gb < G && kdone < T1) {
+                const int rem = gb - 1 - s;
+                const int nk = (T1 - kdone + rem - 1) / rem;
+                kdone += nk;
+                for (int t = 0; t < nk; ++t) {
+                    mbar_wait(&full[stage], par);
+                    const double* sb = stg + stage * LD_STAGE;
+                    const double* as = sb + lc * LD_LDA1 + w1m + lr;
+                    const double* bs = sb + LD_BK * LD_LDA1 + lc * LD_LDB1 + w1n + lr;
+#pragma unroll
+                    for (int ks = 0; ks < LD_BK / 4; ++ks) {
+                        double a[4], bb[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) a[i] = as[ks * 4 * LD_LDA1 + 8 * i];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) bb[j] = bs[ks * 4 * LD_LDB1 + 8 * j];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) dmma884(acc1[i][j][0], acc1[i][j][1], a[i], bb[j]);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[stage]);
+                    if (++stage == LW_ST) { stage = 0; par ^= 1; }
+                }
+            }
+            if (s < 0) continue;
+            const int sl = s & 1;
+            mbar_wait(&wfull[sl], (unsigned)((s >> 1) & 1));
+            const double* Ws = Wsl + sl * LW_WSLOT;
+            for (int u = 0; u < Ct; ++u) {
+                if (u > 0) {                                                  // next tile: up in even steps, down in odd ones
+                    const int prev = (s & 1) ? Ct - u : u - 1;               // live tile before the move
+                    tmem_exchange(tm0 + 64 * ((s & 1) ? prev - 1 : prev), acc2);
+                }
+                for (int t = 0; t < T2; ++t) {
+                    mbar_wait(&full[stage], par);
+                    const double* sb = stg + stage * LD_STAGE;
+                    const double* ws = Ws + (w2m + lr) * LD_LDW + t * LD_BK + lc;
+                    const double* xs = sb + lc * LDX2 + w2n + lr;
+#pragma unroll
+                    for (int ks = 0; ks < LD_BK / 4; ++ks) {
+                        double a[4], bb[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) a[i] = ws[8 * i * LD_LDW + ks * 4];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) bb[j] = xs[ks * 4 * LDX2 + 8 * j];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) dmma884(acc2[i][j][0], acc2[i][j][1], a[i], bb[j]);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[stage]);
+                    if (++stage == LW_ST) { stage = 0; par ^= 1; }
+                }
+            }
+            // this warp is done with chunk s: arm the slot for chunk s+2 (if it comes from a peer) and release it to its builder
+            if (s + 2 < G) {
+                const int bld = (s + 2) % cl;
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[stage]);
-                if (++stage == LC_ST) { stage = 0; par ^= 1; }
+                if (tid == 0 && bld != rank) mbar_expect_tx(&wfull[sl], LW_WSLOT * 8);
+                if (lane == 0) mbar_arrive_cluster(map_shared(&credit[sl], (unsigned)bld));
             }
         }
-        // every CTA has finished reading Ps of this chunk (barrier [1]); my next partial may overwrite it now
-        if (more) publish();
-    }
-    if (has_col) {
+        // write the Ct tiles: the live one first, then continue the alternating walk
         double* Yout = g.nsplit > 1 ? g.Ypart + (long long)split * g.nA * g.nB * g.ldY : g.Y;
+        for (int u = 0; u < Ct; ++u) {
+            const bool down = (G & 1) == 0 ? false : true;                    // step G would walk down if G is odd
+            int tile;
+            if (u > 0) {
+                const int prev = down ? Ct - u : u - 1;
+                tmem_exchange(tm0 + 64 * (down ? prev - 1 : prev), acc2);
+            }
+            tile = down ? Ct - 1 - u : u;
+            const int x0 = (ct0 + tile) * NT2;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int row = w2m + 8 * i + lr;
-            const int p = p0 + row / LD_PQ, q = q0 + row % LD_PQ;
-            if (p >= g.nA || q >= g.nB) continue;
-            double* y = Yout + ((long long)p * g.nB + q) * g.ldY;
+            for (int i = 0; i < 4; ++i) {
+                const int row = w2m + 8 * i + lr;
+                const int p = p0 + row / LD_PQ, q = q0 + row % LD_PQ;
+                if (p >= g.nA || q >= g.nB) continue;
+                double* y = Yout + ((long long)p * g.nB + q) * g.ldY;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < 4; ++j)
 #pragma unroll
-                for (int c = 0; c < 2; ++c) {
-                    const int x = x0 + w2n + 8 * j + 2 * lc + c;
-                    if (x < g.N2) y[x] = acc2[i][j][c];
-                }
+                    for (int c = 0; c < 2; ++c) {
+                        const int x = x0 + w2n + 8 * j + 2 * lc + c;
+                        if (x < g.N2) y[x] = acc2[i][j][c];
+                    }
+            }
         }
     }
-    }
-    // no CTA may retire while a sibling can still touch its shared memory
-    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    // no CTA may retire while a sibling can still copy into its shared memory or arrive on its barriers
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();
+    if (warp == 8) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
 }
 
 // Y = sum over slices of Ypart (fixed order)
@@ -500,65 +611,65 @@ __global__ void ladder_reduce_kernel(const LadderBatch b)
     }
 }
 
-// SMs that clusters of cl CTAs of the wide kernel can keep busy at once (0: size not schedulable); cached per size
-inline int ladder_cluster_active_sms(int cl, int num_sms)
+// SMs that clusters of cl CTAs of the wide kernel can keep busy at once (0: size not schedulable)
+struct LadderOcc { int act[17]; };
+inline void ladder_probe_occupancy(LadderOcc& o, int num_sms)
 {
-    static int tab[17] = {0};
-    static bool done = false;
-    if (!done) {
-        for (int c = 2; c <= 16; ++c) {
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3((unsigned)c * 64); cfg.blockDim = dim3(LD_NTH); cfg.dynamicSmemBytes = ladder_cluster_smem();
-            cudaLaunchAttribute at[1];
-            at[0].id = cudaLaunchAttributeClusterDimension;
-            at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-            cfg.attrs = at; cfg.numAttrs = 1;
-            int n = 0;
-            if (cudaOccupancyMaxActiveClusters(&n, ladder_cluster_kernel, &cfg) == cudaSuccess && n > 0) tab[c] = n * c;
-            cudaGetLastError();
-        }
-        done = true;
+    for (int c = 0; c <= 16; ++c) o.act[c] = 0;
+    for (int c = 1; c <= 16; ++c) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)c * 64); cfg.blockDim = dim3(LW_NTH); cfg.dynamicSmemBytes = ladder_wide_smem();
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)c; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, ladder_wide_kernel, &cfg) == cudaSuccess && n > 0) o.act[c] = n * c > num_sms ? num_sms : n * c;
+        cudaGetLastError();
     }
-    int a = (cl >= 2 && cl <= 16) ? tab[cl] : 0;
-    return a > num_sms ? num_sms : a;
+    if (o.act[1] <= 0) o.act[1] = num_sms;
 }
-// cluster size for ncol column tiles: minimise  groups * (W1 + cl * W2) / active SMs   (W1: building one W chunk,
-// W2: applying it to one column tile); a cluster never spans more column tiles than there are
-inline int ladder_choose_cluster(int ncol, int NQ, int num_sms)
+// Cluster size and column groups for ncol column tiles.  A CTA holds at most LW_MAXC tiles; the W chunks are rebuilt once per
+// group, so the fewest groups win, then the estimated time  (W1 + cl * ceil(tiles / cl) * W2) / active SMs  per row tile and
+// chunk (W1: building one chunk, W2: applying it to one column tile; the busiest CTA of the cluster sets the pace).
+struct LadderTune { int max_cluster = 16, force_cluster = 0, max_tiles = LW_MAXC, force_split = 0; };
+inline void ladder_choose_cluster(int ncol, int NQ, const LadderOcc& occ, const LadderTune& tune, int& cl_out, int& ngrp_out)
 {
-    int maxc = 16;
-    if (const char* e = getenv("RTCC_MAX_CLUSTER")) { int v = atoi(e); if (v >= 2 && v < maxc) maxc = v; }
     const double W1 = 128.0 * 64.0 * NQ, W2 = 64.0 * 128.0 * 128.0;
-    int best = 0; double bt = 1e300;
-    for (int cl = 2; cl <= maxc; ++cl) {
-        const int act = ladder_cluster_active_sms(cl, num_sms);
-        if (act <= 0) continue;
-        const int ngrp = (ncol + cl - 1) / cl;
-        const int ceff = (ncol + ngrp - 1) / ngrp;          // balanced groups
-        if (ceff != cl && cl <= ncol) continue;             // evaluate each balanced size once
-        const double t = ngrp * (W1 + ceff * W2) / ladder_cluster_active_sms(ceff, num_sms);
-        if (ladder_cluster_active_sms(ceff, num_sms) > 0 && t < bt) { bt = t; best = ceff; }
+    int maxc = 16, minc = 1;
+    if (tune.max_cluster >= 1 && tune.max_cluster < maxc) maxc = tune.max_cluster;
+    if (tune.force_cluster >= 1 && tune.force_cluster <= 16 && occ.act[tune.force_cluster] > 0) minc = maxc = tune.force_cluster;
+    const int maxt = tune.max_tiles >= 1 && tune.max_tiles < LW_MAXC ? tune.max_tiles : LW_MAXC;
+    for (int ngrp = 1; ngrp <= ncol; ++ngrp) {
+        const int ng = (ncol + ngrp - 1) / ngrp;            // tiles of the largest group
+        int best = 0; double bt = 1e300;
+        for (int cl = minc; cl <= maxc; ++cl) {
+            if (occ.act[cl] <= 0 || (long long)cl * maxt < ng) continue;
+            const int per = (ng + cl - 1) / cl;
+            const double t = (W1 + (double)cl * per * W2) / occ.act[cl];
+            if (t < bt * (1.0 - 1e-9)) { bt = t; best = cl; }
+        }
+        if (best > 0) { cl_out = best; ngrp_out = ngrp; return; }
     }
-    return best > 0 ? best : 2;
+    cl_out = 1; ngrp_out = (ncol + maxt - 1) / maxt;
 }
 
-// Host side: choose column tile width, cluster shape and the (e,f) slicing so that the items fill the SMs evenly.
-inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
+// Host side: column tile width, cluster shape and (e,f) slicing per spin case.  Narrow cases (one column tile) run in the batched
+// kernel, wide ones in the tensor-memory kernel; max_split bounds the (e,f) slices (each slice needs a partial output buffer).
+inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const LadderOcc& occ, const LadderTune& tune)
 {
     long long rows = 0;
     for (int i = 0; i < b.ncase; ++i) {
         LadderCase& g = b.c[i];
         g.nt2 = g.N2 <= 64 ? 64 : 128;
         g.ncol = (g.N2 + g.nt2 - 1) / g.nt2;
-        g.cl = 1; g.ngrp = g.ncol;
-        if (g.ncol > 1) {                    // balanced groups of at most max_cluster column tiles
-            g.cl = ladder_choose_cluster(g.ncol, b.NQ, num_sms);
-            g.ngrp = (g.ncol + g.cl - 1) / g.cl;
-        }
-        rows += (long long)g.ntiles * g.ngrp * g.cl;
+        g.cl = 0; g.ngrp = 1;                 // cl = 0: batched narrow kernel
+        if (g.ncol > 1) ladder_choose_cluster(g.ncol, b.NQ, occ, tune, g.cl, g.ngrp);
+        else rows += g.ntiles;
     }
+    // narrow cases: slices so that the items fill the SMs evenly
     int best = 1;
-    if (rows < 8LL * num_sms) {
+    if (rows > 0 && rows < 8LL * num_sms) {
         double beff = 0.0;
         for (int S = 1; S <= max_split; ++S) {
             double w = (double)rows * S / num_sms;
@@ -566,16 +677,49 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split)
             if (eff > beff + 0.02) { beff = eff; best = S; }
         }
     }
-    if (const char* e = getenv("RTCC_LADDER_SPLIT")) { int v = atoi(e); if (v >= 1) best = v; }   // tuning knob
+    if (tune.force_split >= 1) best = tune.force_split;
     int item = 0;
     for (int i = 0; i < b.ncase; ++i) {
         LadderCase& g = b.c[i];
         const int nchunk = ((g.vA + LD_PE - 1) / LD_PE) * ((g.vB + LD_PF - 1) / LD_PF);
-        g.nsplit = best < nchunk ? best : (nchunk > 0 ? nchunk : 1);
-        g.item0 = item;
-        if (g.cl == 1) item += g.ntiles * g.ncol * g.nsplit;     // only single-column cases run in the batched kernel
+        g.item0 = 0;
+        if (g.cl == 0) {
+            g.nsplit = best < nchunk ? best : (nchunk > 0 ? nchunk : 1);
+            g.item0 = item;
+            item += g.ntiles * g.ncol * g.nsplit;
+        }
     }
     b.nitems = item;
+    // wide cases: launches are grouped by cluster size; slices only when a launch has few waves
+    for (int i = 0; i < b.ncase; ++i) {
+        LadderCase& g = b.c[i];
+        if (g.cl == 0) continue;
+        bool first = true;
+        for (int k = 0; k < i; ++k) first &= b.c[k].cl != g.cl;
+        if (!first) continue;
+        long long clusters = 0;
+        for (int k = i; k < b.ncase; ++k) if (b.c[k].cl == g.cl) clusters += (long long)b.c[k].ntiles * b.c[k].ngrp;
+        const int conc = occ.act[g.cl] / g.cl > 0 ? occ.act[g.cl] / g.cl : 1;
+        int S = 1;
+        if (clusters < 8LL * conc) {
+            double beff = 0.0;
+            for (int T = 1; T <= max_split; ++T) {
+                double w = (double)clusters * T / conc;
+                double eff = w / ceil(w);
+                if (eff > beff + 0.02) { beff = eff; S = T; }
+            }
+        }
+        if (tune.force_split >= 1) S = tune.force_split;
+        int it = 0;
+        for (int k = i; k < b.ncase; ++k) {
+            LadderCase& h = b.c[k];
+            if (h.cl != g.cl) continue;
+            const int nchunk = ((h.vA + LD_PE - 1) / LD_PE) * ((h.vB + LD_PF - 1) / LD_PF);
+            h.nsplit = S < nchunk ? S : (nchunk > 0 ? nchunk : 1);
+            h.item0 = it;
+            it += h.ntiles * h.ngrp * h.nsplit;
+        }
+    }
 }
 
 // executed tensor-pipe flops of one evaluation
@@ -585,7 +729,7 @@ inline double ladder_flops(const LadderBatch& b)
     for (int i = 0; i < b.ncase; ++i) {
         const LadderCase& g = b.c[i];
         double rows = 64.0 * g.ntiles, ef = (double)g.vA * g.vB;
-        f += 2.0 * rows * ef * ((double)b.NQ * g.ngrp * (g.cl == 1 ? 1.0 : 1.0) + (double)g.ncol * g.nt2);
+        f += 2.0 * rows * ef * ((double)b.NQ * g.ngrp + (double)g.ncol * g.nt2);
     }
     return f;
 }
@@ -595,26 +739,33 @@ inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
     int launches = 0;
     bool red = false;
     if (b.nitems > 0) {
-        LadderBatch pb = b;                       // cluster cases take no items of the batched kernel
-        for (int i = 0; i < pb.ncase; ++i) if (pb.c[i].cl > 1) pb.c[i].ntiles = 0;
-        // (item0 offsets were computed with the cluster cases contributing zero items)
+        LadderBatch pb = b;                       // wide cases take no items of the batched kernel
+        for (int i = 0; i < pb.ncase; ++i) if (pb.c[i].cl > 0) pb.c[i].ntiles = 0;
         ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(pb);
         ++launches;
     }
     for (int i = 0; i < b.ncase; ++i) {
         const LadderCase& g = b.c[i];
         red |= g.nsplit > 1;
-        if (g.cl <= 1 || g.ntiles <= 0) continue;
+        if (g.cl <= 0 || g.ntiles <= 0) continue;
+        bool first = true;
+        for (int k = 0; k < i; ++k) first &= b.c[k].cl != g.cl;
+        if (!first) continue;
+        LadderWide w;
+        w.ncase = 0; w.NQ = b.NQ; w.cl = g.cl;
+        long long clusters = 0;
+        for (int k = i; k < b.ncase; ++k)
+            if (b.c[k].cl == g.cl && b.c[k].ntiles > 0) { w.c[w.ncase++] = b.c[k]; clusters += (long long)b.c[k].ntiles * b.c[k].ngrp * b.c[k].nsplit; }
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)((long long)g.ntiles * g.ngrp * g.nsplit * g.cl));
-        cfg.blockDim = dim3(LD_NTH);
-        cfg.dynamicSmemBytes = ladder_cluster_smem();
+        cfg.gridDim = dim3((unsigned)(clusters * g.cl));
+        cfg.blockDim = dim3(LW_NTH);
+        cfg.dynamicSmemBytes = ladder_wide_smem();
         cfg.stream = st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = (unsigned)g.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, ladder_cluster_kernel, g, b.NQ);
+        cudaLaunchKernelEx(&cfg, ladder_wide_kernel, w);
         ++launches;
     }
     if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); ++launches; }
@@ -625,9 +776,9 @@ inline cudaError_t ladder_init()
 {
     cudaError_t e = cudaFuncSetAttribute(ladder_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_smem());
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(ladder_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_cluster_smem());
+    e = cudaFuncSetAttribute(ladder_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ladder_wide_smem());
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(ladder_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    return cudaFuncSetAttribute(ladder_wide_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
 }
 
 }  // namespace rtcc

@@ -17,6 +17,14 @@
 
 using namespace rtcc;
 
+// process-wide defaults read by rtcc_create (rtcc_set_default_option, include/rtcc.h)
+struct RtccOptions {
+    int fused = 1, fused_fock = 1, graph = 1, prio = 1, tile = 0;
+    LadderTune lad;
+};
+static RtccOptions g_opt;
+static int g_create_cuda_err = 0;            // cudaError_t of the most recent failed rtcc_create
+
 struct rtcc_ctx {
     Dims d{};
     unsigned flags = 0;
@@ -43,6 +51,8 @@ struct rtcc_ctx {
     int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
     int ntiles_ab = 0, ntiles_ss[2]{};
     LadderBatch lb{};
+    LadderOcc locc{};
+    RtccOptions opt{};
     double* ws = nullptr; long long ws_cap = 0;
     double *partial = nullptr, *bmax = nullptr, *scal = nullptr;   // scal: [0..1] E, [2] delta
     double* h_scal = nullptr;                                      // pinned host mirror of scal
@@ -120,7 +130,7 @@ void run(rtcc_ctx* c, TcGemm& g)
 #endif
     const long long cap = c->ws_cap / 8;
     g.ws = c->ws + c->si * cap;
-    int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops);
+    int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops, c->opt.tile);
     c->launches += n;
 }
 inline int nblk(long long n, int cap) { long long b = (n + 255) / 256; if (b < 1) b = 1; if (b > cap) b = cap; return (int)b; }
@@ -699,7 +709,25 @@ const char* rtcc_strerror(int code)
     }
 }
 
-int rtcc_last_cuda_error(const rtcc_ctx* c) { return c ? c->cuda_err : 0; }
+int rtcc_last_cuda_error(const rtcc_ctx* c) { return c ? c->cuda_err : g_create_cuda_err; }
+
+int rtcc_set_default_option(const char* name, int value)
+{
+    if (!name) return RTCC_EINVAL;
+    const std::string k(name);
+    if (k == "fused") g_opt.fused = value != 0;
+    else if (k == "fused_fock") g_opt.fused_fock = value != 0;
+    else if (k == "graph") g_opt.graph = value != 0;
+    else if (k == "stream_priorities") g_opt.prio = value != 0;
+    else if (k == "gemm_tile") { if (value != 0 && value != 64 && value != 128) return RTCC_EINVAL; g_opt.tile = value; }
+    else if (k == "ladder_split") { if (value < 0 || value > 64) return RTCC_EINVAL; g_opt.lad.force_split = value; }
+    else if (k == "max_cluster") { if (value < 1 || value > 16) return RTCC_EINVAL; g_opt.lad.max_cluster = value; }
+    else if (k == "ladder_cluster") { if (value < 0 || value > 16) return RTCC_EINVAL; g_opt.lad.force_cluster = value; }
+    else if (k == "ladder_tiles") { if (value < 1 || value > LW_MAXC) return RTCC_EINVAL; g_opt.lad.max_tiles = value; }
+    else if (k == "reset") g_opt = RtccOptions();
+    else return RTCC_EINVAL;
+    return RTCC_OK;
+}
 
 void rtcc_destroy(rtcc_ctx* c)
 {
@@ -726,6 +754,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
     if (!c) return RTCC_ENOMEM;
     c->flags = flags;
     c->st = (cudaStream_t)cuda_stream;
+    c->opt = g_opt;
     int rc = RTCC_OK;
 #define FAIL(code) do { rc = (code); goto fail; } while (0)
 #define CKC(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { c->cuda_err = (int)e_; rc = RTCC_ECUDA; goto fail; } } while (0)
@@ -751,7 +780,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
         CKC(tcgemm_init());
         CKC(ladder_init());
-        if (dress_smem(d) <= 200 * 1024 && !getenv("RTCC_NO_FUSED")) {
+        if (dress_smem(d) <= 200 * 1024 && c->opt.fused) {
             CKC(cudaFuncSetAttribute(k_dress, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dress_smem(d)));
             c->fused_dress = true;
             // dressed Fock / F / singles fused kernels: per-thread element counts and shared memory must fit
@@ -766,7 +795,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 CKC(cudaFuncSetAttribute(k_postm_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_postp));
                 c->fuse_nch = NQ < 74 ? NQ : 74;
                 c->fuse_sz = (long long)vm * vm + (long long)om * om + (long long)om * vm;
-                c->fused_fock = !getenv("RTCC_NO_FUSED_FOCK");
+                c->fused_fock = c->opt.fused_fock != 0;
             }
         }
         CKC(cudaEventCreate(&c->ev[0]));
@@ -775,7 +804,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         {   // helper branches: everything latency-bound outranks the SM-filling ladder branch (aux[2] = S[3])
             int lo = 0, hi = 0;
             CKC(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-            const bool prio = !getenv("RTCC_NO_PRIO");
+            const bool prio = c->opt.prio != 0;
             for (int i = 0; i < 7; ++i)
                 CKC(cudaStreamCreateWithPriority(&c->aux[i], cudaStreamNonBlocking, (prio && i != 2) ? hi : lo));
         }
@@ -914,7 +943,8 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
-            ladder_plan(B, c->num_sms, 8);
+            ladder_probe_occupancy(c->locc, c->num_sms);
+            ladder_plan(B, c->num_sms, 8, c->locc, c->opt.lad);
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;
@@ -968,7 +998,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             if (read_scal(c)) { rc = RTCC_ECUDA; goto fail; }
             c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
         }
-        if (!getenv("RTCC_NO_GRAPH")) {
+        if (c->opt.graph) {
             cudaStream_t cs = nullptr;
             cudaStream_t user = c->st;
             CKC(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
@@ -993,6 +1023,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
     *out = c;
     return RTCC_OK;
 fail:
+    g_create_cuda_err = c->cuda_err;
     cudaGetLastError();
     rtcc_destroy(c);
     return rc;
@@ -1156,6 +1187,15 @@ int rtcc_ladder_timing(const rtcc_ctx* c, double* ms, double* flops, double* mod
     if (ms) *ms = c->lad_ms;
     if (flops) *flops = c->lad_flops;
     if (model_flops) *model_flops = c->lad_model;
+    return RTCC_OK;
+}
+
+int rtcc_ladder_plan(const rtcc_ctx* c, int spin_case, int out[8])
+{
+    if (!c || !out || spin_case < 0 || spin_case >= c->lb.ncase) return RTCC_EINVAL;
+    const LadderCase& g = c->lb.c[spin_case];
+    out[0] = g.N2; out[1] = g.nt2; out[2] = g.ncol; out[3] = g.cl; out[4] = g.ngrp; out[5] = g.nsplit; out[6] = g.ntiles;
+    out[7] = g.cl > 0 ? c->locc.act[g.cl] : c->num_sms;
     return RTCC_OK;
 }
 

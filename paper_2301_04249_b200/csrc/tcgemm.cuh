@@ -335,7 +335,7 @@ template <int BM, int BN> constexpr size_t tcgemm_smem()
 }
 
 // Host launcher.  ws_cap = capacity (doubles) of g.ws; returns number of kernels launched (1 or 2).
-inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sms, double* flops_out = nullptr)
+inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sms, double* flops_out = nullptr, int force_tile = 0)
 {
     if (g.M <= 0 || g.N <= 0 || g.nb <= 0 || g.nsb <= 0) return 0;
     if (g.Mlo <= 0 || g.Mlo >= g.M) g.Mlo = 0x40000000;
@@ -348,12 +348,8 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     // 128x128 tiles only when they fill the machine at least twice over; below that the 64x64 tiles (3 CTAs per SM, less
     // padding) measured faster (Small: ring products of dimension 907)
     bool big = t128 >= 2LL * num_sms && g.M > 64 && g.N > 64;
-    {   // debugging override: RTCC_TILE=64 / 128 forces a tile configuration
-        static int forced = -1;
-        if (forced < 0) { const char* e = getenv("RTCC_TILE"); forced = e ? atoi(e) : 0; }
-        if (forced == 64) big = false;
-        if (forced == 128) big = true;
-    }
+    if (force_tile == 64) big = false;            // rtcc_set_default_option("tile", ...): tests pin a tile configuration
+    if (force_tile == 128) big = true;
     const int BM = big ? 128 : 64, BN = big ? 128 : 64;
     const long long tiles = (long long)((g.M + BM - 1) / BM) * ((g.N + BN - 1) / BN) * nbt;
     const int nkt = (g.K + 15) / 16;

@@ -22,6 +22,7 @@ SYMBOLS = [
     "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
     "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
+    "rtcc_set_default_option", "rtcc_ladder_plan",
 ]
 
 
@@ -61,6 +62,8 @@ def load():
         lib.rtcc_debug_gemm.argtypes = [i, i, i, vp, vp, vp, d, d, i]
         lib.rtcc_build_fock.argtypes = [i, i, vp, vp, i, i, vp, ctypes.c_uint, vp]
         lib.rtcc_spectral_function.argtypes = [i, d, vp, d, d, d, i, vp, vp, vp]
+        lib.rtcc_set_default_option.argtypes = [ctypes.c_char_p, i]
+        lib.rtcc_ladder_plan.argtypes = [vp, i, P(i)]
         lib.rtcc_last_cuda_error.argtypes = [vp]
         lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
         _lib = lib
@@ -69,6 +72,13 @@ def load():
 
 def strerror(code: int) -> str:
     return load().rtcc_strerror(int(code)).decode()
+
+
+def set_default_option(name: str, value: int = 0):
+    """Process-wide tuning default for contexts created afterwards (include/rtcc.h: rtcc_set_default_option)."""
+    rc = load().rtcc_set_default_option(name.encode(), int(value))
+    if rc:
+        raise RtccError(rc, f"rtcc_set_default_option({name})")
 
 
 def _is_torch(x):
@@ -159,7 +169,7 @@ class Rtcc:
         rc = lib.rtcc_create(ctypes.byref(h), oa, ob, va, vb, n_chol, _ptr(L), _ptr(fock), flags,
                              ctypes.c_void_p(stream or 0))
         if rc:
-            raise RtccError(rc, "rtcc_create")
+            raise RtccError(rc, "rtcc_create", lib.rtcc_last_cuda_error(None))
         self._h = h
         a, b, w = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong()
         lib.rtcc_sizes(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(w))
@@ -250,6 +260,17 @@ class Rtcc:
         a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
         self._ck(self._lib.rtcc_ladder_timing(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "rtcc_ladder_timing")
         return a.value, b.value, c.value
+
+    def ladder_plan(self):
+        """Per spin case with a non-empty block: dict of the pp-ladder launch plan (include/rtcc.h: rtcc_ladder_plan)."""
+        keys = ("columns", "tile", "col_tiles", "cluster", "groups", "ef_slices", "row_tiles", "active_sms")
+        out = []
+        for k in range(3):
+            buf = (ctypes.c_int * 8)()
+            if self._lib.rtcc_ladder_plan(self._h, k, buf):
+                break
+            out.append(dict(zip(keys, list(buf))))
+        return out
 
     def debug_buffer(self, name: str) -> np.ndarray:
         n = self._lib.rtcc_debug_buffer(self._h, name.encode(), None, 0)

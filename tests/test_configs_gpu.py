@@ -1,0 +1,173 @@
+"""BASELINE.json configs 3-5 (Mid / Large / Largest) at FULL size on the literal generator, in the launch
+configuration bench.py times (device pointers, CUDA-graph replay): residual elements placed on the kernels' seams are compared
+one by one with the sampled-element oracle (oracle/rtcc_sampled.c, pinned to the full oracle), E likewise; then the step
+check SURVEY.md 8(c) "Oracle tiers" prescribes: a few Adams-Moulton steps with a fixed micro-iteration count, the update of
+Eq. 9 and the cumulant quadrature (Eq. 5) recomputed on the CPU from downloaded amplitudes.
+Tolerance: BASELINE.json's |dr| <= 1e-10 max|r| per residual element, 1e-8 relative on C."""
+import time
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2301_04249_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-10
+CTOL = 1e-8
+
+
+@pytest.fixture(scope="module")
+def rtcc():
+    from paper_2301_04249_b200 import build, rtcc as m
+    build.build()
+    return m
+
+
+def placed_samples(d, n_random, seed):
+    """Spin-orbital (i, j, a, b) of residual elements chosen on purpose:
+    - ladder row tiles are 8 x 8 blocks of ALL-orbital rows (p, q) = (o+a, o+b): first tile, last (ragged) tile, both sides of
+      a tile boundary, p-tile == q-tile in the same-spin blocks;
+    - ladder / amplitude column tiles are 128 Re|Im-stacked occupied pairs: one element per column tile, so every CTA of a
+      cluster and every parked accumulator tile is hit (pair x lands in tile x/128 with its real and (n_pairs+x)/128 with its
+      imaginary part);
+    - pair-space (ring) tiles are 128 x 128 / 64 x 64 blocks of the (i,a) x (j,b) matrices: first and last rows and columns;
+    plus seeded random draws from each spin block."""
+    oa, ob, va, vb = d.oa, d.ob, d.va, d.vb
+    rng = np.random.default_rng(seed)
+    out = []
+    # alpha-beta block: (i alpha, J beta, a alpha, B beta)
+    noo = oa * ob
+    cols = sorted(set([0, noo - 1] + [min(noo - 1, 128 * k + 5) for k in range((noo + 127) // 128)] + [max(0, noo - 1 - 128 * k) for k in range((noo + 127) // 128)]))
+    rows = [(0, 0), (va - 1, vb - 1), (0, vb - 1), (va - 1, 0), ((8 - oa) % 8, (8 - ob) % 8 + 8), (va // 2, vb // 2 + 1)]
+    for k, x in enumerate(cols):
+        a, B = rows[k % len(rows)]
+        out.append((x // ob, oa + x % ob, min(a, va - 1), va + min(B, vb - 1)))
+    for (a, B) in rows:
+        x = int(rng.integers(0, noo))
+        out.append((x // ob, oa + x % ob, min(a, va - 1), va + min(B, vb - 1)))
+    # same-spin blocks: (i<j, a<b)
+    for s, (o, v, io, iv) in enumerate(((oa, va, 0, 0), (ob, vb, oa, va))):
+        if o < 2 or v < 2:
+            continue
+        npo = o * (o - 1) // 2
+        t0 = (8 - o) % 8                          # first virtual index that starts a row tile
+        ab = [(0, 1), (v - 2, v - 1), (0, v - 1), (t0, t0 + 1), (t0 + 7, t0 + 8), (v // 2, v // 2 + 9)]
+        pcs = sorted(set([0, npo - 1] + [min(npo - 1, 128 * k + 3) for k in range((npo + 127) // 128)]))
+        for k, x in enumerate(pcs):
+            j = int((1 + np.sqrt(1 + 8 * x)) // 2)
+            while j * (j - 1) // 2 > x:
+                j -= 1
+            while (j + 1) * j // 2 <= x:
+                j += 1
+            i = x - j * (j - 1) // 2
+            a, b = ab[k % len(ab)]
+            a, b = max(0, min(a, v - 2)), max(1, min(b, v - 1))
+            if a >= b:
+                a = b - 1
+            out.append((io + i, io + j, iv + a, iv + b))
+    # random draws
+    for _ in range(n_random):
+        blk = int(rng.integers(0, 3))
+        if blk == 2 or oa < 2 or ob < 2:
+            out.append((int(rng.integers(0, oa)), oa + int(rng.integers(0, ob)), int(rng.integers(0, va)), va + int(rng.integers(0, vb))))
+        else:
+            o, v, io, iv = ((oa, va, 0, 0), (ob, vb, oa, va))[blk]
+            i, j = sorted(rng.choice(o, 2, replace=False))
+            a, b = sorted(rng.choice(v, 2, replace=False))
+            out.append((io + int(i), io + int(j), iv + int(a), iv + int(b)))
+    seen, uniq = set(), []
+    for q in out:
+        if q not in seen:
+            seen.add(q); uniq.append(q)
+    return uniq
+
+
+def run_config(rtcc, name, amp_std, n_random, n_r1, max_samples=None, steps=0):
+    import torch
+    from oracle.sampled import SampledOracleC
+    cfg = inputs.CONFIGS[name]
+    t0 = time.time()
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg)                        # literal generator, sigma = 0.3
+    t1, t2 = inputs.random_amplitudes(cfg, std=amp_std)
+    Ld, fd = torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda()
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, Ld, fd)
+    del Ld
+    torch.cuda.empty_cache()
+    t1d, t2d = torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda()
+    r1d, r2d = ctx.residual(t1d, t2d)
+    torch.cuda.synchronize()
+    t_gpu = time.time() - t0
+    r1, r2 = r1d.cpu().numpy(), r2d.cpu().numpy()
+    E = ctx.residual_energy()
+    assert np.isfinite(r1.view(float)).all() and np.isfinite(r2.view(float)).all()
+    scale = max(np.abs(r1).max(), np.abs(r2).max())
+    t0 = time.time()
+    so = SampledOracleC(oa, ob, va, vb, K, L, fock, t1, t2)
+    d = so.d
+    picks = placed_samples(d, n_random, seed=4250 + cfg.index)
+    if max_samples:
+        picks = picks[:max_samples]
+    worst = 0.0
+    for (i, j, a, b) in picks:
+        k = so.packed_of_so_t2(i, j, a, b)
+        assert so.so_of_packed_t2(k) == (i, j, a, b)
+        worst = max(worst, abs(so.r2(i, j, a, b) - r2[k]))
+    rng = np.random.default_rng(77 + cfg.index)
+    for k in [0, d.n_t1 - 1, oa * va - 1, oa * va] + list(rng.integers(0, d.n_t1, n_r1)):
+        i, a = so.so_of_packed_t1(int(k))
+        worst = max(worst, abs(so.r1(i, a) - r1[int(k)]))
+    Eo = so.energy()
+    print(f"{name}: {len(picks)} R2 + {n_r1 + 4} R1 sampled elements, worst |dr| = {worst:.3e}, max|r| = {scale:.3e}, "
+          f"ratio {worst / scale:.2e}; |dE| = {abs(E - Eo):.2e}; gpu {t_gpu:.0f} s, oracle {time.time() - t0:.0f} s, "
+          f"workspace {ctx.workspace_bytes / 2 ** 30:.1f} GiB")
+    assert worst <= RTOL * scale, (worst, scale)
+    assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
+    so.close()
+
+    if steps:
+        # Adams-Moulton step check with downloaded amplitudes (SURVEY.md 8(c) "Oracle tiers"): start from the seeded amplitudes,
+        # fixed_micro = 2.  x0 = t;  B = x0 + h R(x0);  x1 = B + h R(x0);  x2 = B + h R(x1);  C += h (E(x0) + E(x2)),  h = i dt/2.
+        # R(.) on the right-hand sides is the library's residual at the downloaded iterates (its parity is the test above);
+        # what is checked here is the update, the iteration bookkeeping and the quadrature.
+        from oracle.sampled import SampledOracleC as SO
+        h = 0.5j * cfg.dt
+        ctx.set_solver(mode=0, tol=1e-4, max_micro=50, fixed_micro=2)
+        ctx.set_amplitudes(t1d, t2d, 0.0, 0j)
+        C_ref, x1_, x2_ = 0j, t1.copy(), t2.copy()
+        E_prev = E
+        for _ in range(steps):
+            ra, rb = ctx.residual(torch.from_numpy(x1_).cuda(), torch.from_numpy(x2_).cuda())
+            B1, B2 = x1_ + h * ra.cpu().numpy(), x2_ + h * rb.cpu().numpy()
+            y1, y2 = B1 + h * ra.cpu().numpy(), B2 + h * rb.cpu().numpy()
+            ra, rb = ctx.residual(torch.from_numpy(y1).cuda(), torch.from_numpy(y2).cuda())
+            x1_, x2_ = B1 + h * ra.cpu().numpy(), B2 + h * rb.cpu().numpy()
+            assert ctx.step(cfg.dt) == 2
+            g1, g2 = ctx.get_amplitudes()
+            g1, g2 = g1.cpu().numpy(), g2.cpu().numpy()
+            amax = max(np.abs(x2_).max(), np.abs(x1_).max())
+            assert np.abs(g2 - x2_).max() <= 1e-13 * amax and np.abs(g1 - x1_).max() <= 1e-13 * amax
+            x1_, x2_ = g1, g2
+            so = SO(oa, ob, va, vb, K, L, fock, x1_, x2_)
+            E_new = so.energy()
+            so.close()
+            C_ref += h * (E_prev + E_new)
+            E_prev = E_new
+            C, Eg = ctx.cumulant()
+            assert abs(Eg - E_new) <= RTOL * max(1.0, abs(E_new))
+            assert abs(C - C_ref) <= CTOL * abs(C_ref)
+        print(f"{name}: {steps} Adams-Moulton steps (fixed_micro 2): C = {C:.12e}, oracle-side C = {C_ref:.12e}")
+    ctx.close()
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("amp_std", [1e-3, 3e-2])
+def test_residual_mid_config_sampled(rtcc, amp_std):
+    """Config 3 (o=24, v=200, n_chol=900): general tcgemm path (no fused small kernels), 128 x 128 tiles at scale, the wide ladder."""
+    run_config(rtcc, "mid", amp_std, n_random=10, n_r1=6, steps=2 if amp_std == 1e-3 else 0)
+
+
+def test_residual_large_config_sampled(rtcc):
+    """Config 4 (o=40, v=360, n_chol=1600): 3120 stacked amplitude columns."""
+    run_config(rtcc, "large", 1e-3, n_random=4, n_r1=3, max_samples=26)

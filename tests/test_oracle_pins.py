@@ -392,6 +392,58 @@ def test_sampled_oracle_matches_full_oracle():
         assert abs(so.r2(j, i, a, b) + so.r2(i, j, a, b)) < 1e-13
 
 
+def test_sampled_c_oracle_matches_full_oracle():
+    """rtcc_sampled.c (the tier-B oracle that fits configs 3-5) against tier A: EVERY packed element of R1 and R2 and E, complex
+    amplitudes, general Fock matrix, shapes with o_s in {0, 1}, v_s = 1 and unequal spins; then spin-orbital elements outside
+    the packed set (antisymmetric partners, a spin-forbidden one) to pin the accessors' sign and spin rules."""
+    from oracle.sampled import SampledOracleC
+    shapes = [(2, 3, 4, 3, 5, 21), (3, 1, 2, 4, 4, 22), (2, 2, 3, 3, 6, 23), (2, 0, 3, 5, 4, 24), (1, 2, 2, 1, 3, 25), (3, 3, 5, 5, 7, 26)]
+    for (oa, ob, va, vb, K, seed) in shapes:
+        L, fock = rand_problem(oa, ob, va, vb, K, seed)
+        prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+        t1p, t2p = rand_amps(prob.d, seed + 100)
+        r1p, r2p, E = prob.residual(t1p, t2p)
+        scale = max(np.abs(r2p).max(initial=0), np.abs(r1p).max(initial=0), 1.0)
+        so = SampledOracleC(oa, ob, va, vb, K, L, fock, t1p, t2p)
+        assert abs(so.energy() - E) < 1e-13 * max(1.0, abs(E))
+        for k in range(prob.d.n_t2):
+            i, j, a, b = so.so_of_packed_t2(k)
+            assert so.packed_of_so_t2(i, j, a, b) == k
+            assert abs(so.r2(i, j, a, b) - r2p[k]) < 2e-13 * scale, (k, i, j, a, b)
+        for k in range(prob.d.n_t1):
+            i, a = so.so_of_packed_t1(k)
+            assert abs(so.r1(i, a) - r1p[k]) < 2e-13 * scale
+        if prob.d.n_t2:
+            t1, t2 = orc.unpack(prob.d, t1p, t2p)
+            r1so, r2so, _ = prob.residual_so(t1, t2)
+            i, j, a, b = so.so_of_packed_t2(prob.d.n_t2 - 1)
+            for (p, q, r, s) in ((j, i, a, b), (i, j, b, a), (j, i, b, a)):
+                assert abs(so.r2(p, q, r, s) - r2so[p, q, r, s]) < 2e-13 * scale
+            if oa and ob:
+                assert so.r2(0, oa, 0, 1 if va > 1 else 0) == 0 or va == 1      # (alpha beta | alpha alpha): spin-forbidden
+        so.close()
+
+
+def test_sampled_c_oracle_matches_numpy_sampled_oracle_beyond_tier_a():
+    """A size the full oracle cannot hold comfortably (N = 60 spin-orbitals): the two independently written sampled oracles
+    (numpy einsum vs C loops) agree on a spread of elements from all three spin blocks."""
+    from oracle.sampled import SampledOracle, SampledOracleC
+    oa, ob, va, vb, K = 4, 5, 26, 25, 31
+    L, fock = rand_problem(oa, ob, va, vb, K, 41)
+    d = orc.Dims(oa, ob, va, vb, K)
+    t1p, t2p = rand_amps(d, 141)
+    a_, c_ = SampledOracle(oa, ob, va, vb, K, L, fock, t1p, t2p), SampledOracleC(oa, ob, va, vb, K, L, fock, t1p, t2p)
+    assert abs(a_.energy() - c_.energy()) < 1e-12
+    rng = np.random.default_rng(5)
+    for k in list(rng.integers(0, d.n_t2, 12)) + [0, d.n_t2 - 1]:
+        idx = a_.so_of_packed_t2(int(k))
+        assert abs(a_.r2(*idx) - c_.r2(*idx)) < 1e-12 * max(1.0, abs(a_.r2(*idx)))
+    for k in (0, d.n_t1 - 1, d.n_t1 // 2):
+        idx = a_.so_of_packed_t1(int(k))
+        assert abs(a_.r1(*idx) - c_.r1(*idx)) < 1e-12
+    c_.close()
+
+
 # ------------------------------------------------------------------ NEXT-3: (N-1) Fock matrix, PAPER.md:48
 def test_fock_n1_is_eps_minus_antisymmetrised_core_integral():
     """f_pq = eps_p delta_pq - <pc||qc>: the per-spin Coulomb/exchange formula must equal the spin-orbital definition

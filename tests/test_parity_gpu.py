@@ -70,6 +70,54 @@ def test_residual_general_fock_complex_amplitudes(rtcc, shape):
     check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
 
 
+@pytest.mark.parametrize("opts", [
+    {"ladder_cluster": 2}, {"ladder_cluster": 3}, {"ladder_cluster": 5}, {"ladder_cluster": 4, "ladder_split": 3},
+    {"ladder_tiles": 1}, {"ladder_tiles": 2, "ladder_cluster": 2}, {"ladder_tiles": 1, "max_cluster": 2}, {"ladder_split": 2},
+])
+def test_wide_ladder_cluster_shapes(rtcc, opts):
+    """The wide ladder kernel's code paths that the automatic plan picks only at larger sizes, forced on a size the full oracle
+    checks element by element: W chunks exchanged between the CTAs of a cluster (2, 3, 4, 5 CTAs: even and odd cluster sizes use
+    the two shared-memory slots differently), CTAs with fewer column tiles than their siblings (5 tiles over 2 / 3 / 4 CTAs),
+    several column groups (tiles per CTA capped at 1 or 2, cluster capped at 2: W rebuilt per group), and (e,f)
+    slices with partial outputs."""
+    oa, ob, va, vb, K = 17, 16, 19, 20, 23          # widths 544 (ab: 5 tiles), 272 / 240 (aa, bb: 3 / 2 tiles); 3 x 3 (e,f) chunks
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=55)
+    d = orc.Dims(oa, ob, va, vb, K)
+    rng = np.random.default_rng(9)
+    t1 = 0.1 * (rng.standard_normal(d.n_t1) + 1j * rng.standard_normal(d.n_t1))
+    t2 = 0.1 * (rng.standard_normal(d.n_t2) + 1j * rng.standard_normal(d.n_t2))
+    global _WIDE_REF
+    key = "ref"
+    if key not in _WIDE_REF:
+        prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+        _WIDE_REF[key] = prob.residual(t1, t2)
+    r1o, r2o, Eo = _WIDE_REF[key]
+    try:
+        for k, v in opts.items():
+            rtcc.set_default_option(k, v)
+        ctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)
+        plan = ctx.ladder_plan()
+        r1, r2 = ctx.residual(t1, t2)
+        ra, rb = ctx.residual(t1, t2)
+        ctx.close()
+    finally:
+        rtcc.set_default_option("reset")
+    scale = max(np.abs(r1o).max(), np.abs(r2o).max())
+    assert np.abs(r2 - r2o).max() <= RTOL * scale and np.abs(r1 - r1o).max() <= RTOL * scale
+    assert np.array_equal(r2, rb) and np.array_equal(r1, ra)          # bit-reproducible
+    assert [p["col_tiles"] for p in plan] == [5, 3, 2]
+    if "ladder_cluster" in opts:
+        assert all(p["cluster"] == opts["ladder_cluster"] for p in plan)
+    if "ladder_tiles" in opts:
+        assert all(p["groups"] * p["cluster"] * opts["ladder_tiles"] >= p["col_tiles"] for p in plan)
+        assert plan[0]["groups"] > 1 or plan[0]["cluster"] * opts["ladder_tiles"] >= 5
+    if "ladder_split" in opts:
+        assert all(p["ef_slices"] == opts["ladder_split"] for p in plan)
+
+
+_WIDE_REF = {}
+
+
 def test_residual_tiny_config_literal_generator(rtcc):
     """BASELINE.json config 1 (Tiny): literal generator, seeded N(0,1e-3) complex amplitudes and t = 0."""
     cfg = inputs.CONFIGS["tiny"]
@@ -233,7 +281,7 @@ def test_residual_small_config_full_size_sampled(rtcc, amp_std):
     assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
 
 
-def test_general_gemm_path_without_fused_small_kernels(rtcc, monkeypatch):
+def test_general_gemm_path_without_fused_small_kernels(rtcc):
     """The fused small-problem kernels (k_dress, k_fock_*, k_postm_*) replace tcgemm launches only when a slice fits in
     shared memory; the general path must give the same residual (it is the one larger configurations run)."""
     oa, ob, va, vb, K = 5, 4, 18, 19, 37
@@ -242,11 +290,18 @@ def test_general_gemm_path_without_fused_small_kernels(rtcc, monkeypatch):
     rng = np.random.default_rng(8)
     t1 = 0.1 * (rng.standard_normal(d.n_t1) + 1j * rng.standard_normal(d.n_t1))
     t2 = 0.1 * (rng.standard_normal(d.n_t2) + 1j * rng.standard_normal(d.n_t2))
-    monkeypatch.setenv("RTCC_NO_FUSED", "1")
-    check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
-    monkeypatch.delenv("RTCC_NO_FUSED")
-    monkeypatch.setenv("RTCC_NO_FUSED_FOCK", "1")
-    check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+    try:
+        rtcc.set_default_option("fused", 0)
+        check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+        rtcc.set_default_option("reset")
+        rtcc.set_default_option("fused_fock", 0)
+        check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+        rtcc.set_default_option("reset")
+        rtcc.set_default_option("graph", 0)
+        rtcc.set_default_option("gemm_tile", 128)
+        check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+    finally:
+        rtcc.set_default_option("reset")
 
 
 def test_build_fock_matches_oracle(rtcc):
