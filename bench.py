@@ -1,14 +1,16 @@
 #!/usr/bin/env python
-"""bench.py -- RT-EOM-CCSD time-steps/s on BASELINE.json's configs[1] ("small": 8 occupied, 60 virtual, n_chol 340).
+"""bench.py -- RT-EOM-CCSD time-steps/s on BASELINE.json's configs[2] ("mid": 24 occupied, 200 virtual, n_chol 900), the
+largest configuration whose 20-step run fits the driver's time box; Small and one Large residual ride along in `per_config`.
 
-A "step" is one pass of the whole hot path: one rtcc_step = first-order Adams-Moulton step (Eq. 9)
-with its fixed-point micro-iterations, each a full evaluation of the complex spin-explicit CCSD right-hand side
-(Eqs. 7-8) from the Cholesky vectors, plus the cumulant update (Eq. 5).  Prints ONE JSON line (see DESIGN.md
-section 8 for every key).  `--impl reference` times the CPU oracle instead (a deliberately plain program).
+A "step" is one pass of the whole hot path: one rtcc_step = first-order Adams-Moulton step (Eq. 9) with its
+fixed-point micro-iterations, each a full evaluation of the complex spin-explicit CCSD right-hand side (Eqs. 7-8) from the
+Cholesky vectors, plus the cumulant update (Eq. 5).  Prints ONE JSON line (DESIGN.md section 8 explains every key).
+`--impl reference` times the CPU oracle instead (a deliberately plain program) on a bounded sample of the same generator.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
 import subprocess
@@ -25,58 +27,74 @@ from paper_2301_04249_b200 import inputs  # noqa: E402
 
 METRIC = "rt_eom_ccsd_time_steps_per_s"
 UNIT = "steps/s"
-# solver settings of the timed workload: the paper's plain fixed-point iteration of Eq. 9 with the
-# paper's cutoff 1e-4.  The literal sigma=0.3 generator of BASELINE.json diverges in the second step at
-# this size, so the timed propagation uses the stabilised scale sigma_s = 0.2*sqrt(144/(v*d))
-# (same shapes, same flops per residual; a documented deviation).
+# Solver of the timed workload: the paper's plain fixed-point iteration of Eq. 9 with a
+# FIXED number of micro-iterations per step, so that the work per step is defined: at dt = 0.05 the plain
+# iteration contracts at ~0.84 per sweep from the orbital-energy diagonal alone (core level at -20 Ha), i.e. ~50 sweeps to the
+# paper's 1e-4 cutoff.  The amplitudes stay finite at the stabilised scale sigma_s; flops per residual
+# do not depend on values.
 BENCH_MODE = 0
 BENCH_TOL = 1e-4
-BENCH_FIXED_MICRO = 0
+BENCH_FIXED_MICRO = 4
 L2_BYTES = 126 * 2 ** 20
-LADDER_DRAM_BYTES_NCU = 92.7e6      # per launch, workload 'small' (profiles/r01d_topkernel_ncu.md: 65.2 MB read + 27.4 MB written)
+CONFIG_INDEX = {"tiny": 0, "small": 1, "mid": 2, "large": 3, "largest": 4}
+# the oracle sample both the cpu_baseline leg and --impl reference time: same generator family, small enough that one
+# Adams-Moulton step (1 + fixed_micro residual evaluations of the naive spin-orbital oracle) takes a few seconds
+SAMPLE_O, SAMPLE_V, SAMPLE_K = 4, 30, 170
 
 
 def mac_model(o, v):
-    """Naive spin-orbital ladder MAC count o_so^2 v_so^4 used to scale the oracle sample."""
-    return (2.0 * o) ** 2 * (2.0 * v) ** 4
+    """Naive spin-orbital ladder MAC count o_so^2 v_so^4 that dominates the oracle's residual."""
+    return (2.0 * o - 1.0) ** 2 * (2.0 * v + 1.0) ** 4
 
 
-def oracle_sample_rate(cfg_full, sample_cfg, fixed_micro, n_steps, warmup):
-    """Times the oracle, as it stands, on a reduced problem of the same generator; returns
-    (steps/s extrapolated to cfg_full, threads, description, measured s/step on the sample)."""
+def solver_text(mode, fixed):
+    what = "plain Eq. 9 fixed point (PAPER.md:103)" if mode == 0 else "denominator-preconditioned fixed point (NEXT-1)"
+    return f"mode {mode} ({what}), " + (f"fixed_micro {fixed} (exactly {fixed} micro-iterations per step)" if fixed else f"tol {BENCH_TOL} (PAPER.md:139)")
+
+
+def oracle_sample_rate(cfg_full, n_steps, warmup, mode, fixed_micro):
+    """Times the full spin-orbital oracle, as it stands, on a reduced problem of the same generator (stabilised sigma, same
+    solver settings); returns (steps/s scaled to cfg_full by the o_so^2 v_so^4 MAC count, threads, description, measured s/step,
+    scale factor)."""
     from oracle import oracle as orc
-    oa, ob, va, vb, K, L, fock = inputs.make_problem(sample_cfg, sigma=inputs.stabilised_sigma(sample_cfg))
+    sample = inputs.custom(SAMPLE_O, SAMPLE_V, SAMPLE_K, d=cfg_full.d * SAMPLE_K / cfg_full.K, v_lo=cfg_full.v_lo, v_hi=cfg_full.v_hi,
+                           dt=cfg_full.dt, index=cfg_full.index, name=cfg_full.name + "-sample")
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(sample, sigma=inputs.stabilised_sigma(sample))
     prob = orc.Problem(oa, ob, va, vb, K, L, fock)
-    prop = orc.Propagator(prob, mode=BENCH_MODE, tol=BENCH_TOL, max_micro=200, fixed_micro=fixed_micro)
+    prop = orc.Propagator(prob, mode=mode, tol=BENCH_TOL, max_micro=200, fixed_micro=fixed_micro)
     for _ in range(warmup):
-        prop.step(sample_cfg.dt)
+        prop.step(sample.dt)
     t0 = time.perf_counter()
     micro = 0
     for _ in range(n_steps):
-        micro += prop.step(sample_cfg.dt)
+        micro += prop.step(sample.dt)
     dt = (time.perf_counter() - t0) / max(n_steps, 1)
-    scale = mac_model(cfg_full.o, cfg_full.v) / mac_model(sample_cfg.o, sample_cfg.v)
-    desc = (f"oracle AM1 steps (mode {BENCH_MODE}, tol {BENCH_TOL}, {micro / max(n_steps, 1):.1f} micro-iterations/step) on the same "
-            f"generator (stabilised sigma) at o={sample_cfg.o}, "
-            f"v={sample_cfg.v}, n_chol={sample_cfg.K}: {dt:.3f} s/step measured over {n_steps} steps, scaled x{scale:.0f} by the "
-            f"o_so^2 v_so^4 MAC count to o={cfg_full.o}, v={cfg_full.v} (extrapolated)")
-    return 1.0 / (dt * scale), orc.num_threads(), desc, dt
+    scale = mac_model(cfg_full.o, cfg_full.v) / mac_model(sample.o, sample.v)
+    desc = (f"full spin-orbital oracle (oracle/rtcc_oracle.c, naive loops, OpenMP), Adams-Moulton steps with {solver_text(mode, fixed_micro)}, "
+            f"{micro / max(n_steps, 1):.1f} micro-iterations/step, on the same generator (stabilised sigma) at o={sample.o}, v={sample.v}, "
+            f"n_chol={sample.K}: {dt:.3f} s/step measured over {n_steps} steps after {warmup} warm-up step(s); scaled x{scale:.3g} by the "
+            f"o_so^2 v_so^4 MAC count to o={cfg_full.o}, v={cfg_full.v} (EXTRAPOLATED: the oracle's 4-index tensor does not fit beyond config 2)")
+    return 1.0 / (dt * scale), orc.num_threads(), desc, dt, scale
+
+
+def workload_text(cfg, dims):
+    oa, ob, va, vb = dims
+    return (f"BASELINE.json configs[{CONFIG_INDEX.get(cfg.name, '?')}] '{cfg.name}' (o={cfg.o}, v={cfg.v}, n_chol={cfg.K}, dt={cfg.dt}, "
+            f"o_a/o_b/v_a/v_b={oa}/{ob}/{va}/{vb}), seeded generator at the stabilised scale sigma_s = 0.2*sqrt(144/(v*d)) "
+            f"(BASELINE.json's literal 0.3 is not propagatable, BASELINE.md section 4), state from T=0")
 
 
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    frac = 3.0 / 8.0
-    sample = inputs.custom(max(2, round(cfg.o * frac)), round(cfg.v * frac), round(cfg.K * frac), d=cfg.d, v_lo=cfg.v_lo,
-                           v_hi=cfg.v_hi, dt=cfg.dt, index=cfg.index, name=cfg.name + "-sample")
-    value, cores, desc, s_per = oracle_sample_rate(cfg, sample, BENCH_FIXED_MICRO, args.steps, args.warmup)
+    value, cores, desc, s_per, scale = oracle_sample_rate(cfg, args.steps, args.warmup, args.mode, args.fixed_micro)
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[1] '{cfg.name}' (o={cfg.o}, v={cfg.v}, n_chol={cfg.K}, dt={cfg.dt})",
-                   "solver": f"mode {BENCH_MODE} (plain Eq. 9), tol {BENCH_TOL}"},
+        "warmup": args.warmup, "ms_per_step": 1e3 * s_per, "ms_per_step_note": "measured per step of the bounded SAMPLE; value = 1 / (that x extrapolation_factor)",
+        "extrapolation_factor": scale,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_text(cfg, cfg.dims), "solver": solver_text(args.mode, args.fixed_micro)},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -104,7 +122,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                       "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.p = None
 
@@ -117,21 +135,111 @@ class ClockSampler:
         except Exception:
             self.p.kill()
             out = ""
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in out.strip().splitlines():
             f = [x.strip() for x in line.split(",")]
             if len(f) < 7:
                 continue
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
             except ValueError:
                 continue
             for nm, val in zip(names, f[3:7]):
                 if val.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def residual_model_flops(oa, ob, va, vb, K):
+    """F_model of SURVEY.md 8(d): real x real MAC = 2 flops, real x complex = 4, complex x complex = 8."""
+    P = lambda x: x * (x - 1) / 2.0
+    pp_apply = 4.0 * (P(va) ** 2 * P(oa) + P(vb) ** 2 * P(ob) + (va * vb) ** 2 * oa * ob)
+    pp_build = 2.0 * K * (2 * P(va) ** 2 + 2 * P(vb) ** 2 + (va * vb) ** 2)
+    hh = 12.0 * (P(oa) ** 2 * P(va) + P(ob) ** 2 * P(vb) + (oa * ob) ** 2 * va * vb)
+    n1, nA, nB = oa * va + ob * vb, oa * vb, ob * va
+    ring = 12.0 * (float(n1) ** 3 + float(nA) * nB * nB + float(nB) * nA * nA)      # the 10 spin-pattern GEMMs
+    chol = 12.0 * K * (oa * va + ob * vb) ** 2 + 8.0 * K * (oa + ob) * (va ** 2 + vb ** 2)
+    return pp_apply + pp_build + hh + ring + chol
+
+
+def load_profile(name):
+    """ncu figures of the dominant kernel come from a committed summary under profiles/ (never typed into this file)."""
+    best = None
+    for p in sorted(glob.glob(os.path.join(ROOT, "profiles", "*.json"))):
+        try:
+            j = json.load(open(p))
+        except Exception:
+            continue
+        if j.get("workload") == name and j.get("kernel", "").startswith("ladder"):
+            best = (p, j)
+    return best
+
+
+def measure_residual(ctx, rtcc, cfg, flush, stream, reps):
+    """Device time of one residual evaluation (graph replay) and of the pp-ladder launches inside it (timing mode)."""
+    import torch
+    t1, t2 = inputs.random_amplitudes(cfg)
+    t1d, t2d = torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda()
+    r1d, r2d = torch.empty_like(t1d), torch.empty_like(t2d)
+    ctx.set_timing(True)
+    lad = []
+    for i in range(reps + 1):
+        flush.fill_(i)
+        ctx.residual(t1d, t2d, r1d, r2d)
+        lad.append(ctx.ladder_timing())
+    ctx.set_timing(False)
+    lad_ms = float(np.mean([x[0] for x in lad[1:]]))
+    ctx.residual(t1d, t2d, r1d, r2d)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        ctx.residual(t1d, t2d, r1d, r2d)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ctx.reset_counters()
+    ctx.residual(t1d, t2d, r1d, r2d)
+    launches, exec_flops = ctx.counters()
+    finite = bool(torch.isfinite(torch.view_as_real(r2d)).all())
+    return {"res_ms": e0.elapsed_time(e1) / reps, "lad_ms": lad_ms, "lad_exec": lad[-1][1], "lad_model": lad[-1][2],
+            "launches": launches, "exec_flops": exec_flops, "finite": finite}
+
+
+def config_block(rtcc, name, stream, flush, peak, with_steps):
+    """One entry of `per_config`: residual time / model rate / ladder fraction of another BASELINE.json config."""
+    import torch
+    cfg = inputs.CONFIGS[name]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=inputs.stabilised_sigma(cfg))
+    Ld = torch.from_numpy(L).cuda()
+    del L
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, Ld, torch.from_numpy(fock).cuda(), stream=stream.cuda_stream)
+    del Ld
+    torch.cuda.empty_cache()
+    m = measure_residual(ctx, rtcc, cfg, flush, stream, 2 if name in ("large", "largest") else 5)
+    f_model = residual_model_flops(oa, ob, va, vb, K)
+    out = {"workload": workload_text(cfg, (oa, ob, va, vb)), "residual_ms": m["res_ms"], "residual_model_tflops": f_model / m["res_ms"] * 1e-9,
+           "residual_pct_of_fp64_peak": 100.0 * f_model / m["res_ms"] * 1e-9 / peak, "ladder_ms": m["lad_ms"],
+           "ladder_model_tflops": m["lad_model"] / m["lad_ms"] * 1e-9, "ladder_frac": m["lad_model"] / m["lad_ms"] * 1e-9 / peak,
+           "ladder_executed_tflops": m["lad_exec"] / m["lad_ms"] * 1e-9, "ladder_plan": ctx.ladder_plan(),
+           "launches_per_residual": m["launches"], "workspace_bytes": ctx.workspace_bytes, "finite": m["finite"]}
+    if with_steps:
+        ctx.set_solver(mode=BENCH_MODE, tol=BENCH_TOL, max_micro=200, fixed_micro=0)
+        for _ in range(3):
+            ctx.step(cfg.dt)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        micro = 0
+        for _ in range(with_steps):
+            micro += ctx.step(cfg.dt)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        out["steps_per_s"] = with_steps / (e0.elapsed_time(e1) * 1e-3)
+        out["solver"] = solver_text(BENCH_MODE, 0)
+        out["micro_iters_per_step"] = micro / with_steps
+    ctx.close()
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args, cfg):
@@ -157,7 +265,7 @@ def run_ours(args, cfg):
     stream = torch.cuda.current_stream()
     Ld, fd = torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda()
     ctx = rtcc.Rtcc(oa, ob, va, vb, K, Ld, fd, stream=stream.cuda_stream)
-    ctx.set_solver(mode=BENCH_MODE, tol=BENCH_TOL, max_micro=200, fixed_micro=BENCH_FIXED_MICRO)
+    ctx.set_solver(mode=args.mode, tol=BENCH_TOL, max_micro=200, fixed_micro=args.fixed_micro)
     flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device="cuda")
 
     def sync_all():
@@ -178,136 +286,124 @@ def run_ours(args, cfg):
         micro += ctx.step(cfg.dt)
         evs[s][1].record(stream)
     sync_all()
-    launches, flops = ctx.counters()
+    launches, _ = ctx.counters()
     clocks = sampler.stop() if sampler else None
     ms = sum(a.elapsed_time(b) for a, b in evs)
     ms_total, value = aggregate_replicas(ms, args.steps, world, dist, device="cuda")
     C, E = ctx.cumulant()
 
-    # dominant kernel: the chained pp-ladder (3 launches per residual), timed live with CUDA events on the stream
-    t1, t2 = inputs.random_amplitudes(cfg)
-    t1d, t2d = torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda()
-    r1d, r2d = torch.empty_like(t1d), torch.empty_like(t2d)
-    ctx.set_timing(True)
-    lad = []
-    for i in range(6):
-        flush.fill_(i)
-        ctx.residual(t1d, t2d, r1d, r2d)
-        lad.append(ctx.ladder_timing())
-    ctx.set_timing(False)
-    lad_ms = float(np.mean([x[0] for x in lad[1:]]))
-    lad_exec, lad_model = lad[-1][1], lad[-1][2]
+    # dominant kernel: the chained pp-ladder, timed live with CUDA events on the stream; whole residual by graph replay
+    m = measure_residual(ctx, rtcc, cfg, flush, stream, 3)
     peak = rtcc.fp64_peak()
-    # whole-residual device time (graph replay) for the model TFLOP/s of the residual
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ctx.residual(t1d, t2d, r1d, r2d)
-    e0.record(stream)
-    for _ in range(5):
-        ctx.residual(t1d, t2d, r1d, r2d)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    res_ms = e0.elapsed_time(e1) / 5
     f_model = residual_model_flops(oa, ob, va, vb, K)
+    plan = ctx.ladder_plan()
+    wide = any(p["cluster"] > 0 for p in plan)
 
     # end to end through the C ABI with HOST buffers: each step the amplitudes come from pinned host memory
     # (rtcc_set_amplitudes: H2D + R(t)), rtcc_step, and go back (rtcc_get_amplitudes: D2H) with C(t)
-    e2e = None
-    if True:
-        hctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock, stream=stream.cuda_stream)
-        hctx.set_solver(mode=BENCH_MODE, tol=BENCH_TOL, max_micro=200, fixed_micro=BENCH_FIXED_MICRO)
-        n1, n2 = hctx.n_t1, hctx.n_t2
-        h1 = torch.zeros(n1, dtype=torch.complex128).pin_memory().numpy()
-        h2 = torch.zeros(n2, dtype=torch.complex128).pin_memory().numpy()
-        Ch, tm = 0j, 0.0
-        nst = max(3, min(args.steps, 10))
-        for it in range(2 + nst):
-            if it == 2:
-                sync_all()
-                t0 = time.perf_counter()
-            hctx.set_amplitudes(h1, h2, tm, Ch)
-            hctx.step(cfg.dt)
-            a1, a2 = hctx.get_amplitudes()
-            h1[:] = a1; h2[:] = a2
-            Ch, _ = hctx.cumulant(); tm = hctx.time
-        torch.cuda.synchronize()
-        el = time.perf_counter() - t0
-        tt = torch.tensor([el], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * nst / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": 16 * (n1 + n2),
-               "d2h_bytes_per_step": 16 * (n1 + n2) + 32, "steps": nst,
-               "what": "per step: rtcc_set_amplitudes(host)+rtcc_step+rtcc_get_amplitudes(host)+rtcc_cumulant, RTCC_HOST_PTRS context"}
-        hctx.close()
+    hctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock, stream=stream.cuda_stream)
+    hctx.set_solver(mode=args.mode, tol=BENCH_TOL, max_micro=200, fixed_micro=args.fixed_micro)
+    n1, n2 = hctx.n_t1, hctx.n_t2
+    h1 = torch.zeros(n1, dtype=torch.complex128).pin_memory().numpy()
+    h2 = torch.zeros(n2, dtype=torch.complex128).pin_memory().numpy()
+    Ch, tm = 0j, 0.0
+    nst = max(3, min(args.steps, 5 if cfg.name != "small" else 10))
+    for it in range(1 + nst):
+        if it == 1:
+            sync_all()
+            t0 = time.perf_counter()
+        hctx.set_amplitudes(h1, h2, tm, Ch)
+        hctx.step(cfg.dt)
+        a1, a2 = hctx.get_amplitudes()
+        h1[:] = a1; h2[:] = a2
+        Ch, _ = hctx.cumulant(); tm = hctx.time
+    torch.cuda.synchronize()
+    el = time.perf_counter() - t0
+    tt = torch.tensor([el], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    e2e = {"value": world * nst / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": 16 * (n1 + n2),
+           "d2h_bytes_per_step": 16 * (n1 + n2) + 32, "steps": nst,
+           "what": "per step: rtcc_set_amplitudes(host: H2D + R(t)) + rtcc_step + rtcc_get_amplitudes(host: D2H) + rtcc_cumulant, RTCC_HOST_PTRS context; "
+                   "one residual evaluation more per step than the resident loop (R at the uploaded amplitudes)"}
+    hctx.close()
+    workspace = ctx.workspace_bytes
+    ctx.close()
+    del Ld
+    torch.cuda.empty_cache()
 
     if rank == 0:
         cpu = None
+        per_config = {}
         if world == 1 and not args.no_cpu_baseline:
-            sample = inputs.custom(4, 30, 170, d=cfg.d, v_lo=cfg.v_lo, v_hi=cfg.v_hi, dt=cfg.dt, index=cfg.index)
-            v_, cores, desc, _ = oracle_sample_rate(cfg, sample, BENCH_FIXED_MICRO, 1, 0)
+            v_, cores, desc, _, _ = oracle_sample_rate(cfg, 3, 1, args.mode, args.fixed_micro)
             cpu = {"value": v_, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        if world == 1 and not args.no_per_config:
+            for name in ("small", "large"):
+                if name != cfg.name:
+                    try:
+                        per_config[name] = config_block(rtcc, name, stream, flush, peak, with_steps=20 if name == "small" else 0)
+                    except Exception as e:                                    # e.g. a smaller GPU: report, do not hide
+                        per_config[name] = {"error": str(e)}
+        prof = load_profile(cfg.name)
+        roof = {"bound": "tensor",
+                "kernel": ("ladder_wide_kernel (alpha-beta launch + batched alpha-alpha/beta-beta launch" if wide else "ladder_kernel (ab, aa, bb batched")
+                          + "; W tiles from the Cholesky vectors, never stored)",
+                "achieved": m["lad_model"] / m["lad_ms"] * 1e-9, "peak": peak, "unit": "TFLOP/s",
+                "frac": m["lad_model"] / m["lad_ms"] * 1e-9 / peak,
+                "traffic": prof[1].get("dram_bytes_per_residual") if prof else None,
+                "traffic_source": (os.path.relpath(prof[0], ROOT) + ": " + prof[1].get("source", "")) if prof else None,
+                "ncu_dmma_pipe_active_pct": prof[1].get("dmma_pipe_active_pct") if prof else None,
+                "executed_tflops": m["lad_exec"] / m["lad_ms"] * 1e-9, "ms": m["lad_ms"], "algorithmic_flops": m["lad_model"],
+                "algorithmic_flops_note": "SURVEY.md 8(d): pp apply 4[P(va)^2 P(oa)+P(vb)^2 P(ob)+(va vb)^2 oa ob] + W-build 2K[2P(va)^2+2P(vb)^2+(va vb)^2], per residual",
+                "ladder_plan": plan,
+                "peak_source": "measured live: register-resident FP64 DMMA loop (rtcc_fp64_peak); MEASURED_PEAKS.json has no fp64 figure"}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[1] '{cfg.name}' (o={cfg.o}, v={cfg.v}, n_chol={cfg.K}, dt={cfg.dt}, "
-                                   f"o_a/o_b/v_a/v_b={oa}/{ob}/{va}/{vb}), state from T=0",
-                       "sigma": sigma, "sigma_note": "stabilised scale 0.2*sqrt(144/(v*d)); BASELINE.json's literal 0.3 diverges in step 2 (BASELINE.md section 4)",
-                       "solver": f"mode {BENCH_MODE} ({'plain Eq. 9 fixed point' if BENCH_MODE == 0 else 'denominator-preconditioned fixed point, NEXT-1'}), tol {BENCH_TOL} (PAPER.md:139)",
-                       "micro_iters_per_step": micro / args.steps, "l2": "flushed between timed steps (252 MiB write)",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "workspace_bytes": ctx.workspace_bytes},
-            "residual": {"ms": res_ms, "model_flops": f_model, "model_tflops": f_model / res_ms * 1e-9,
-                         "pct_of_fp64_peak": 100.0 * f_model / res_ms * 1e-9 / peak, "executed_dmma_flops": ctx_res_flops(ctx)},
-            "roofline": {"bound": "tensor", "kernel": "ladder_kernel (one launch per residual: ab, aa, bb spin cases batched)",
-                         "achieved": lad_model / lad_ms * 1e-9, "peak": peak, "unit": "TFLOP/s",
-                         "frac": lad_model / lad_ms * 1e-9 / peak, "traffic": LADDER_DRAM_BYTES_NCU if cfg.name == "small" else None,
-                         "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture (profiles/r01d_topkernel_ncu.md)",
-                         "ncu_dmma_pipe_active_pct": 92.6,
-                         "executed_tflops": lad_exec / lad_ms * 1e-9, "ms": lad_ms, "algorithmic_flops": lad_model,
-                         "peak_source": "measured live: register-resident FP64 DMMA loop (rtcc_fp64_peak); MEASURED_PEAKS.json has no fp64 figure"},
-            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "cumulant": {"re": C.real, "im": C.imag, "time_au": ctx.time},
+            "config": {"workload": workload_text(cfg, (oa, ob, va, vb)), "sigma": sigma,
+                       "solver": solver_text(args.mode, args.fixed_micro),
+                       "micro_iters_per_step": micro / args.steps, "residual_evaluations_per_step": micro / args.steps,
+                       "l2": "flushed between timed steps (252 MiB write); operands of one residual (>= 1 GB) exceed L2 anyway",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "workspace_bytes": workspace},
+            "residual": {"ms": m["res_ms"], "model_flops": f_model, "model_tflops": f_model / m["res_ms"] * 1e-9,
+                         "pct_of_fp64_peak": 100.0 * f_model / m["res_ms"] * 1e-9 / peak, "executed_dmma_flops": m["exec_flops"],
+                         "launches": m["launches"]},
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "per_config": per_config,
+            "cumulant": {"re": C.real, "im": C.imag, "time_au": (args.steps + args.warmup) * cfg.dt},
         }
         print(json.dumps(out))
-    ctx.close()
     if dist is not None:
         dist.destroy_process_group()
-
-
-def ctx_res_flops(ctx):
-    ctx.reset_counters()
-    import torch
-    z1 = torch.zeros(ctx.n_t1, dtype=torch.complex128, device="cuda")
-    z2 = torch.zeros(ctx.n_t2, dtype=torch.complex128, device="cuda")
-    ctx.residual(z1, z2)
-    return ctx.counters()[1]
-
-
-def residual_model_flops(oa, ob, va, vb, K):
-    """F_model of SURVEY.md 8(d): real x real MAC = 2 flops, real x complex = 4, complex x complex = 8."""
-    P = lambda x: x * (x - 1) / 2.0
-    pp_apply = 4.0 * (P(va) ** 2 * P(oa) + P(vb) ** 2 * P(ob) + (va * vb) ** 2 * oa * ob)
-    pp_build = 2.0 * K * (2 * P(va) ** 2 + 2 * P(vb) ** 2 + (va * vb) ** 2)
-    hh = 12.0 * (P(oa) ** 2 * P(va) + P(ob) ** 2 * P(vb) + (oa * ob) ** 2 * va * vb)
-    n1, nA, nB = oa * va + ob * vb, oa * vb, ob * va
-    ring = 12.0 * (float(n1) ** 3 + float(nA) * nB * nB + float(nB) * nA * nA)      # the 10 spin-pattern GEMMs
-    chol = 12.0 * K * (oa * va + ob * vb) ** 2 + 8.0 * K * (oa + ob) * (va ** 2 + vb ** 2)
-    return pp_apply + pp_build + hh + ring + chol
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="small", choices=list(inputs.CONFIGS))
+    ap.add_argument("--config", default="mid", choices=list(inputs.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mode", type=int, default=0, choices=[0, 1],
+    ap.add_argument("--no-per-config", action="store_true", help="skip the Small / Large entries of per_config")
+    ap.add_argument("--mode", type=int, default=BENCH_MODE, choices=[0, 1],
                     help="0: the paper's plain fixed point of Eq. 9 (default, the headline); 1: denominator-preconditioned (NEXT-1)")
+    ap.add_argument("--fixed-micro", type=int, default=None, help="micro-iterations per step (0: iterate to tol 1e-4)")
     args = ap.parse_args()
+    if args.fixed_micro is None:
+        args.fixed_micro = 0 if args.config in ("tiny", "small") else BENCH_FIXED_MICRO
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    globals()["BENCH_MODE"] = args.mode
     cfg = inputs.CONFIGS[args.config]
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and world == 1:
+        # replicas only: one process per GPU; outside torchrun this script starts them itself
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", os.environ.get("MASTER_PORT", "29531"), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if world > 1 and args.gpus != world:
+        raise SystemExit(f"--gpus {args.gpus} does not match WORLD_SIZE {world}")
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -110,6 +110,9 @@ int rtcc_ladder_timing(const rtcc_ctx* ctx, double* ms, double* flops, double* m
  * the last): out = { stacked Re|Im columns, column tile width, column tiles, CTAs per cluster (0: narrow batched kernel),
  * column groups, (e,f) slices, row tiles, SMs the clusters can occupy }. */
 int rtcc_ladder_plan(const rtcc_ctx* ctx, int spin_case, int out[8]);
+/* out[k], k = 1..16: SMs that clusters of k CTAs of the wide ladder kernel can occupy at once on this device (0: not
+ * schedulable), from cudaOccupancyMaxActiveClusters; the plan weighs cluster sizes with it. */
+int rtcc_ladder_occupancy(const rtcc_ctx* ctx, int out[17]);
 
 /* (N-1)-electron Fock matrix from the Cholesky vectors and the orbital energies of the N-electron reference
  * (f_pq = eps_p delta_pq - v_pc^qc, c = core-hole spin-orbital; v_pq^rs = <pq||rs>):

@@ -689,10 +689,12 @@ __global__ void k_caxpy(long long n, const double* __restrict__ a, const double*
 // Adams-Moulton micro-iteration (Eq. 9):
 //   mode 0:  y = B + h R(x)                       h = i dt/2
 //   mode 1:  y = (B + h (R(x) - D x)) / (1 - h D) D = orbital-energy denominator (same fixed point)
-// writes y, and the block maxima of |y - x| (a non-finite value is reported as +inf).
+// writes y, and the block maxima of |y - x| (a non-finite value is reported as +inf).  xin and y MAY BE THE SAME ARRAY (the
+// iterate is updated in place from the second micro-iteration on): neither is __restrict__, each element is read before it
+// is written by the same thread.
 __global__ void __launch_bounds__(RED_THREADS) k_am_update(long long n, const double* __restrict__ Bv, const double* __restrict__ R,
-                                                           const double* __restrict__ xin, const double* __restrict__ Dn, int mode,
-                                                           double dt_half, double* __restrict__ y, double* __restrict__ bmax)
+                                                           const double* xin, const double* __restrict__ Dn, int mode,
+                                                           double dt_half, double* y, double* __restrict__ bmax)
 {
     __shared__ double sh[32];
     double mx = 0.0;

@@ -1199,6 +1199,13 @@ int rtcc_ladder_plan(const rtcc_ctx* c, int spin_case, int out[8])
     return RTCC_OK;
 }
 
+int rtcc_ladder_occupancy(const rtcc_ctx* c, int out[17])
+{
+    if (!c || !out) return RTCC_EINVAL;
+    for (int i = 0; i <= 16; ++i) out[i] = c->locc.act[i];
+    return RTCC_OK;
+}
+
 int rtcc_build_fock(int n, int NQ, const double* L, const double* eps, int cs, int ci, double* fock, unsigned flags, void* stream)
 {
     if (n < 1 || NQ < 1 || !L || !eps || !fock || (cs != 0 && cs != 1) || ci < 0 || ci >= n) return RTCC_EINVAL;

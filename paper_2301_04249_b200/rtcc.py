@@ -22,7 +22,7 @@ SYMBOLS = [
     "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
     "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
-    "rtcc_set_default_option", "rtcc_ladder_plan",
+    "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy",
 ]
 
 
@@ -64,6 +64,7 @@ def load():
         lib.rtcc_spectral_function.argtypes = [i, d, vp, d, d, d, i, vp, vp, vp]
         lib.rtcc_set_default_option.argtypes = [ctypes.c_char_p, i]
         lib.rtcc_ladder_plan.argtypes = [vp, i, P(i)]
+        lib.rtcc_ladder_occupancy.argtypes = [vp, P(i)]
         lib.rtcc_last_cuda_error.argtypes = [vp]
         lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
         _lib = lib
@@ -271,6 +272,11 @@ class Rtcc:
                 break
             out.append(dict(zip(keys, list(buf))))
         return out
+
+    def ladder_occupancy(self):
+        buf = (ctypes.c_int * 17)()
+        self._ck(self._lib.rtcc_ladder_occupancy(self._h, buf), "rtcc_ladder_occupancy")
+        return list(buf)
 
     def debug_buffer(self, name: str) -> np.ndarray:
         n = self._lib.rtcc_debug_buffer(self._h, name.encode(), None, 0)
