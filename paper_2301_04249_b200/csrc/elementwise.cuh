@@ -612,6 +612,7 @@ __global__ void __launch_bounds__(256) k_tsc_matvec(Dims d, const double* __rest
 struct EnergyArgs {
     const double* L[2]; const double* Lt[2]; const double* fock[2];   // bare vectors, dressed vectors (planar), bare Fock
     const double* t1r; const double* Mq; const double* gam; double* partial;   // partial[RED_BLOCKS][2]
+    unsigned* counter; double* out;                                             // last block: out[0..1] = sum of the partials
 };
 
 // E = sum f_ia t_i^a + 1/2 [ sum_Q,ia L_ia M_ia + sum_Q gamma_Q^2 - sum_s sum_Q,ij U_ji U_ij ],  U = L~_oo - L_oo
@@ -661,15 +662,20 @@ __global__ void __launch_bounds__(RED_THREADS) k_energy(Dims d, EnergyArgs A)
     }
     double a = block_sum(sr, sh);
     double b = block_sum(si, sh);
-    if (threadIdx.x == 0) { A.partial[2 * blockIdx.x] = a; A.partial[2 * blockIdx.x + 1] = b; }
-}
-
-__global__ void k_sum_partials(const double* __restrict__ partial, int nblocks, double* __restrict__ out2)
-{
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
-        double a = 0.0, b = 0.0;
-        for (int i = 0; i < nblocks; ++i) { a += partial[2 * i]; b += partial[2 * i + 1]; }
-        out2[0] = a; out2[1] = b;
+    __shared__ bool last;
+    if (threadIdx.x == 0) {
+        A.partial[2 * blockIdx.x] = a; A.partial[2 * blockIdx.x + 1] = b;
+        __threadfence();
+        last = atomicAdd(A.counter, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last) {          // the last block adds the block sums in a fixed order (thread t: blocks t, t + 256, ...; then the block tree)
+        __threadfence();
+        double pa = 0.0, pb = 0.0;
+        for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) { pa += A.partial[2 * i]; pb += A.partial[2 * i + 1]; }
+        pa = block_sum(pa, sh);
+        pb = block_sum(pb, sh);
+        if (threadIdx.x == 0) { A.out[0] = pa; A.out[1] = pb; *A.counter = 0u; }
     }
 }
 
@@ -686,86 +692,126 @@ __global__ void k_caxpy(long long n, const double* __restrict__ a, const double*
     }
 }
 
+// The packed amplitude vector [t1 alpha | t1 beta | aa | bb | ab] as five row x column segments; the orbital-energy
+// denominator of an element is colE[col] - rowE[row] (D_i^a = f_aa - f_ii, D_ij^ab = f_aa + f_bb - f_ii - f_jj), read from
+// small per-segment tables instead of an amplitude-sized array.
+struct AmpSegs {
+    long long off[6];            // segment s holds elements off[s] .. off[s+1]
+    int ncol[5];
+    const double* rowE[5];
+    const double* colE[5];
+};
+// rowE / colE tables (one launch at setup): tab = [oa | ob | po_a | po_b | oa*ob | va | vb | pv_a | pv_b | va*vb]
+__global__ void k_build_denominator_tables(Dims d, const double* __restrict__ f0, const double* __restrict__ f1,
+                                           const int2* __restrict__ op0, const int2* __restrict__ op1,
+                                           const int2* __restrict__ vp0, const int2* __restrict__ vp1, double* __restrict__ tab)
+{
+    const int n = d.n;
+    const long long cnt[10] = {d.o[0], d.o[1], d.po[0], d.po[1], d.oo, d.v[0], d.v[1], d.pv[0], d.pv[1], (long long)d.v[0] * d.v[1]};
+    long long tot = 0;
+    for (int k = 0; k < 10; ++k) tot += cnt[k];
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        long long y = x; int k = 0;
+        while (y >= cnt[k]) { y -= cnt[k]; ++k; }
+        const int oa = d.o[0], ob = d.o[1];
+        auto eo = [&](int s, int i) { const double* f = s ? f1 : f0; return f[(long long)i * n + i]; };
+        auto ev = [&](int s, int a) { const double* f = s ? f1 : f0; const int o = s ? ob : oa; return f[(long long)(o + a) * n + o + a]; };
+        double v;
+        switch (k) {
+            case 0: v = eo(0, (int)y); break;
+            case 1: v = eo(1, (int)y); break;
+            case 2: { int2 ij = op0[y]; v = eo(0, ij.x) + eo(0, ij.y); break; }
+            case 3: { int2 ij = op1[y]; v = eo(1, ij.x) + eo(1, ij.y); break; }
+            case 4: v = eo(0, (int)(y / ob)) + eo(1, (int)(y % ob)); break;
+            case 5: v = ev(0, (int)y); break;
+            case 6: v = ev(1, (int)y); break;
+            case 7: { int2 ab = vp0[y]; v = ev(0, ab.x) + ev(0, ab.y); break; }
+            case 8: { int2 ab = vp1[y]; v = ev(1, ab.x) + ev(1, ab.y); break; }
+            default: v = ev(0, (int)(y / d.v[1])) + ev(1, (int)(y % d.v[1])); break;
+        }
+        tab[x] = v;
+    }
+}
+
 // Adams-Moulton micro-iteration (Eq. 9):
 //   mode 0:  y = B + h R(x)                       h = i dt/2
 //   mode 1:  y = (B + h (R(x) - D x)) / (1 - h D) D = orbital-energy denominator (same fixed point)
-// writes y, and the block maxima of |y - x| (a non-finite value is reported as +inf).  xin and y MAY BE THE SAME ARRAY (the
-// iterate is updated in place from the second micro-iteration on): neither is __restrict__, each element is read before it
-// is written by the same thread.
-__global__ void __launch_bounds__(RED_THREADS) k_am_update(long long n, const double* __restrict__ Bv, const double* __restrict__ R,
-                                                           const double* xin, const double* __restrict__ Dn, int mode,
-                                                           double dt_half, double* y, double* __restrict__ bmax)
+// writes y and the block maxima of |y - x| (a non-finite value is reported as +inf); the last block to finish reduces the
+// block maxima to out_delta[0] (max is order-independent, so this stays bit-reproducible).
+// first != 0: x = t(tau), R = R(t(tau)) and B = t + h R is formed here and stored OVER R (Bv == R): the Adams-Moulton history is
+// then three amplitude-sized vectors (t, B, iterate) plus the residual of the iterate.
+// Aliasing: xin may be y (in-place iterate), Bv may be R (first): none of the four is __restrict__; every element is read
+// before it is written, by the same thread.
+constexpr int AM_CHUNK = 8;
+__global__ void __launch_bounds__(RED_THREADS) k_am_update(long long n, AmpSegs sg, double* Bv, const double* R, const double* xin, int mode, int first,
+                                                           double dt_half, double* y, double* __restrict__ bmax, unsigned* __restrict__ counter,
+                                                           double* __restrict__ out_delta)
 {
     __shared__ double sh[32];
+    __shared__ bool last;
     double mx = 0.0;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n; x += (long long)gridDim.x * blockDim.x) {
-        double2 b = reinterpret_cast<const double2*>(Bv)[x], r = reinterpret_cast<const double2*>(R)[x];
-        double2 t = reinterpret_cast<const double2*>(xin)[x], o;
-        if (mode == 0) {
-            o.x = b.x - dt_half * r.y;
-            o.y = b.y + dt_half * r.x;
-        } else {
-            double D = Dn[x];
-            double gr = r.x - D * t.x, gi = r.y - D * t.y;          // R - D x
-            double nr = b.x - dt_half * gi, ni = b.y + dt_half * gr; // B + h (R - D x)
-            double c = dt_half * D;                                   // 1 - h D = 1 - i c
-            double den = 1.0 / (1.0 + c * c);
-            o.x = (nr - c * ni) * den;                                // (nr + i ni)(1 + i c)/(1+c^2)
-            o.y = (ni + c * nr) * den;
+    const long long per = (long long)RED_THREADS * AM_CHUNK;
+    for (long long c0 = blockIdx.x * per; c0 < n; c0 += (long long)gridDim.x * per) {
+        long long x = c0 + threadIdx.x;
+        int seg = 0; long long row = 0; int col = 0;
+        if (mode != 0 && x < n) {
+            while (x >= sg.off[seg + 1]) ++seg;
+            const long long y0 = x - sg.off[seg];
+            row = y0 / sg.ncol[seg]; col = (int)(y0 - row * sg.ncol[seg]);
         }
-        reinterpret_cast<double2*>(y)[x] = o;
-        double dx = o.x - t.x, dy = o.y - t.y;
-        double a = sqrt(dx * dx + dy * dy);
-        if (!(a == a) || isinf(a)) a = INFINITY;
-        mx = fmax(mx, a);
+#pragma unroll 2
+        for (int j = 0; j < AM_CHUNK; ++j, x += RED_THREADS) {
+            if (x >= n) break;
+            double2 r = reinterpret_cast<const double2*>(R)[x];
+            double2 t = reinterpret_cast<const double2*>(xin)[x], b, o;
+            if (first) {
+                b.x = t.x - dt_half * r.y;
+                b.y = t.y + dt_half * r.x;
+                reinterpret_cast<double2*>(Bv)[x] = b;
+            } else b = reinterpret_cast<const double2*>(Bv)[x];
+            if (mode == 0) {
+                o.x = b.x - dt_half * r.y;
+                o.y = b.y + dt_half * r.x;
+            } else {
+                const double D = sg.colE[seg][col] - sg.rowE[seg][row];
+                double gr = r.x - D * t.x, gi = r.y - D * t.y;          // R - D x
+                double nr = b.x - dt_half * gi, ni = b.y + dt_half * gr; // B + h (R - D x)
+                double c = dt_half * D;                                   // 1 - h D = 1 - i c
+                double den = 1.0 / (1.0 + c * c);
+                o.x = (nr - c * ni) * den;                                // (nr + i ni)(1 + i c)/(1+c^2)
+                o.y = (ni + c * nr) * den;
+                const long long xn = x + RED_THREADS;                     // (segment, row, column) of the next element
+                if (xn < n) {
+                    if (xn >= sg.off[seg + 1] || sg.ncol[seg] < RED_THREADS) {
+                        while (xn >= sg.off[seg + 1]) ++seg;
+                        const long long y0 = xn - sg.off[seg];
+                        row = y0 / sg.ncol[seg]; col = (int)(y0 - row * sg.ncol[seg]);
+                    } else {
+                        col += RED_THREADS;
+                        if (col >= sg.ncol[seg]) { col -= sg.ncol[seg]; ++row; }
+                    }
+                }
+            }
+            reinterpret_cast<double2*>(y)[x] = o;
+            double dx = o.x - t.x, dy = o.y - t.y;
+            double a = sqrt(dx * dx + dy * dy);
+            if (!(a == a) || isinf(a)) a = INFINITY;
+            mx = fmax(mx, a);
+        }
     }
     double m = block_max(mx, sh);
-    if (threadIdx.x == 0) bmax[blockIdx.x] = m;
-}
-
-__global__ void k_max_partials(const double* __restrict__ bmax, int n, double* __restrict__ out)
-{
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
-        double m = 0.0;
-        for (int i = 0; i < n; ++i) m = fmax(m, bmax[i]);
-        out[0] = m;
+    if (threadIdx.x == 0) {
+        bmax[blockIdx.x] = m;
+        __threadfence();
+        last = atomicAdd(counter, 1u) == gridDim.x - 1;
     }
-}
-
-// orbital-energy denominators of every packed element (t1 then t2): D = f_aa (+ f_bb) - f_ii (- f_jj)
-__global__ void k_build_Dn(Dims d, const double* __restrict__ f0, const double* __restrict__ f1,
-                           const int2* __restrict__ op0, const int2* __restrict__ op1,
-                           const int2* __restrict__ vp0, const int2* __restrict__ vp1, double* __restrict__ Dn)
-{
-    const long long nss0 = (long long)d.po[0] * d.pv[0], nss1 = (long long)d.po[1] * d.pv[1];
-    const long long tot = d.n_t1 + d.n_t2;
-    const int n = d.n;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
-        double D;
-        if (x < d.n_t1) {
-            int s = x >= d.n1a; int cc = (int)(s ? x - d.n1a : x);
-            int i = cc / d.v[s], a = cc - i * d.v[s];
-            const double* f = s ? f1 : f0;
-            D = f[(long long)(d.o[s] + a) * n + d.o[s] + a] - f[(long long)i * n + i];
-        } else {
-            long long k = x - d.n_t1;
-            if (k < nss0 + nss1) {
-                int s = k >= nss0; if (s) k -= nss0;
-                int pij = (int)(k / d.pv[s]), pab = (int)(k - (long long)pij * d.pv[s]);
-                int2 ij = (s ? op1 : op0)[pij], ab = (s ? vp1 : vp0)[pab];
-                const double* f = s ? f1 : f0; const int o = d.o[s];
-                D = f[(long long)(o + ab.x) * n + o + ab.x] + f[(long long)(o + ab.y) * n + o + ab.y]
-                  - f[(long long)ij.x * n + ij.x] - f[(long long)ij.y * n + ij.y];
-            } else {
-                k -= nss0 + nss1;
-                int B = (int)(k % d.v[1]); k /= d.v[1];
-                int a = (int)(k % d.v[0]); k /= d.v[0];
-                int J = (int)(k % d.o[1]); int i = (int)(k / d.o[1]);
-                D = f0[(long long)(d.o[0] + a) * n + d.o[0] + a] + f1[(long long)(d.o[1] + B) * n + d.o[1] + B]
-                  - f0[(long long)i * n + i] - f1[(long long)J * n + J];
-            }
-        }
-        Dn[x] = D;
+    __syncthreads();
+    if (last) {
+        __threadfence();
+        double v = 0.0;
+        for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) v = fmax(v, bmax[i]);
+        v = block_max(v, sh);
+        if (threadIdx.x == 0) { out_delta[0] = v; *counter = 0u; }
     }
 }
 

@@ -57,7 +57,9 @@ struct rtcc_ctx {
     double *partial = nullptr, *bmax = nullptr, *scal = nullptr;   // scal: [0..1] E, [2] delta
     double* h_scal = nullptr;                                      // pinned host mirror of scal
     double *gx = nullptr, *gr = nullptr;                           // residual input / output (packed amp vectors)
-    double *t_cur = nullptr, *r_cur = nullptr, *Bv = nullptr, *Dn = nullptr;
+    double *t_cur = nullptr, *r_cur = nullptr;                     // t(tau), R(t(tau)); during a step r_cur holds B = t + h R(t)
+    double* dtab = nullptr; AmpSegs segs{};                        // orbital-energy tables behind the denominators
+    unsigned* counters = nullptr;                                  // [0] energy reduction, [1] update reduction
     double *io = nullptr;                                          // staging for host-pointer mode
     long long namp = 0;                                            // n_t1 + n_t2 (complex)
 
@@ -250,9 +252,9 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         EnergyArgs ea;
         for (int s = 0; s < 2; ++s) { ea.L[s] = c->L[s]; ea.Lt[s] = c->Lt[s]; ea.fock[s] = c->fockd[s]; }
         ea.t1r = c->t1r; ea.Mq = c->Mq; ea.gam = c->gam; ea.partial = c->partial;
+        ea.counter = c->counters; ea.out = c->scal;
         k_energy<<<RED_BLOCKS, RED_THREADS, 0, ST>>>(d, ea);
-        k_sum_partials<<<1, 32, 0, ST>>>(c->partial, RED_BLOCKS, c->scal);
-        c->launches += 2;
+        c->launches += 1;
     }
 
     // ---- 6+7 (fused path for small problems): dressed Fock, F intermediates and singles in seven launches on branch 4
@@ -888,8 +890,8 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->gr, 2 * c->namp, "gr");
         DA(c->t_cur, 2 * c->namp, nullptr);
         DA(c->r_cur, 2 * c->namp, nullptr);
-        DA(c->Bv, 2 * c->namp, nullptr);
-        DA(c->Dn, c->namp, "Dn");
+        DA(c->counters, 4, nullptr);
+        CKC(cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned), c->st));
 
         // inputs
         const cudaMemcpyKind kin = (flags & RTCC_HOST_PTRS) ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -983,7 +985,23 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             ops_rr(g, c->L[1] + ob, c->L[0] + oa, c->KxBA);
             run(c, g);
         }
-        EW(c, k_build_Dn, c->namp, d, c->fockd[0], c->fockd[1], c->opairs[0], c->opairs[1], c->vpairs[0], c->vpairs[1], c->Dn);
+        {   // orbital-energy tables of the five segments of the packed amplitude vector (denominators formed on the fly)
+            const long long cnt[10] = {oa, ob, d.po[0], d.po[1], d.oo, va, vb, d.pv[0], d.pv[1], (long long)va * vb};
+            long long tot = 0, offs[10];
+            for (int k = 0; k < 10; ++k) { offs[k] = tot; tot += cnt[k]; }
+            DA(c->dtab, tot, nullptr);
+            EW(c, k_build_denominator_tables, tot, d, c->fockd[0], c->fockd[1], c->opairs[0], c->opairs[1], c->vpairs[0], c->vpairs[1], c->dtab);
+            AmpSegs& sg = c->segs;
+            const long long len[5] = {(long long)oa * va, (long long)ob * vb, (long long)d.po[0] * d.pv[0], (long long)d.po[1] * d.pv[1], (long long)d.oo * va * vb};
+            const int ncol[5] = {va, vb, d.pv[0], d.pv[1], va * vb};
+            sg.off[0] = 0;
+            for (int k = 0; k < 5; ++k) {
+                sg.off[k + 1] = sg.off[k] + len[k];
+                sg.ncol[k] = ncol[k] > 0 ? ncol[k] : 1;
+                sg.rowE[k] = c->dtab + offs[k];
+                sg.colE[k] = c->dtab + offs[5 + k];
+            }
+        }
         CKC(cudaMemsetAsync(c->t_cur, 0, (size_t)c->namp * 16, c->st));
         CKC(cudaMemsetAsync(c->gx, 0, (size_t)c->namp * 16, c->st));
         model_ladder_flops(c);
@@ -1101,22 +1119,34 @@ int rtcc_set_solver(rtcc_ctx* c, int mode, double tol, int max_micro, int fixed_
     return RTCC_OK;
 }
 
+// restores R(t(tau)) after a failed step (its storage held B): one residual evaluation at the unchanged amplitudes
+static int restore_r_cur(rtcc_ctx* c)
+{
+    CK(cudaMemcpyAsync(c->gx, c->t_cur, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    int rc = eval_gx(c);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return RTCC_OK;
+}
+
 int rtcc_step(rtcc_ctx* c, double dt)
 {
     if (!c || !std::isfinite(dt)) return RTCC_EINVAL;
     const long long N = c->namp;
     const double hh = 0.5 * dt;
-    // B = t + (i dt/2) R(t)
-    k_caxpy<<<nblk(N, c->num_sms * 16), 256, 0, c->st>>>(N, c->t_cur, c->r_cur, 0.0, hh, c->Bv);
-    c->launches++;
     int k = 0;
     double E_new[2] = {0, 0};
+    int fail = RTCC_OK;
     for (;;) {
+        // first micro-iteration: B = t + (i dt/2) R(t) is formed inside the update and stored over R(t); later ones update the
+        // iterate in place.  Three amplitude-sized vectors (t, B, iterate) + the residual of the iterate.
         const double* xin = k == 0 ? c->t_cur : c->gx;
         const double* rin = k == 0 ? c->r_cur : c->gr;
-        k_am_update<<<RED_BLOCKS, RED_THREADS, 0, c->st>>>(N, c->Bv, rin, xin, c->Dn, c->mode, hh, c->gx, c->bmax);
-        k_max_partials<<<1, 32, 0, c->st>>>(c->bmax, RED_BLOCKS, c->scal + 2);
-        c->launches += 2;
+        k_am_update<<<RED_BLOCKS, RED_THREADS, 0, c->st>>>(N, c->segs, c->r_cur, rin, xin, c->mode, k == 0 ? 1 : 0, hh, c->gx, c->bmax,
+                                                           c->counters + 1, c->scal + 2);
+        c->launches += 1;
+        if (cudaGetLastError() != cudaSuccess) { fail = RTCC_ECUDA; break; }
         ++k;
         const bool last_fixed = c->fixed_micro > 0 && k >= c->fixed_micro;
         // The convergence measure is copied back behind the update and the residual R(x_k) -- needed whether or not the
@@ -1127,18 +1157,26 @@ int rtcc_step(rtcc_ctx* c, double dt)
             CK(cudaEventRecord(c->ev_delta, c->st));
         }
         int rc = eval_gx(c);
-        if (rc) return rc;
+        if (rc) { fail = rc; break; }
         if (c->fixed_micro > 0) {
             if (last_fixed) break;
             continue;
         }
         CK(cudaEventSynchronize(c->ev_delta));
-        if (!std::isfinite(c->h_scal[2])) { cudaStreamSynchronize(c->st); return RTCC_ENONFINITE; }
+        if (!std::isfinite(c->h_scal[2])) { fail = RTCC_ENONFINITE; break; }
         if (c->h_scal[2] < c->tol) break;
-        if (k >= c->max_micro) { cudaStreamSynchronize(c->st); return RTCC_ENOCONV; }
+        if (k >= c->max_micro) { fail = RTCC_ENOCONV; break; }
     }
-    if (read_scal(c)) return RTCC_ECUDA;
-    if (!std::isfinite(c->h_scal[2]) || !std::isfinite(c->h_scal[0]) || !std::isfinite(c->h_scal[1])) return RTCC_ENONFINITE;
+    if (!fail) {
+        if (read_scal(c)) fail = RTCC_ECUDA;
+        else if (!std::isfinite(c->h_scal[2]) || !std::isfinite(c->h_scal[0]) || !std::isfinite(c->h_scal[1])) fail = RTCC_ENONFINITE;
+    }
+    if (fail) {                                   // state not advanced: t(tau) is untouched, R(t(tau)) is evaluated again
+        cudaStreamSynchronize(c->st);
+        cudaGetLastError();
+        if (k > 0) { int rc = restore_r_cur(c); if (rc && fail != RTCC_ECUDA) return rc; }
+        return fail;
+    }
     E_new[0] = c->h_scal[0]; E_new[1] = c->h_scal[1];
     // C += (i dt/2) (E_old + E_new)
     const double sr = c->E[0] + E_new[0], si = c->E[1] + E_new[1];
