@@ -41,7 +41,8 @@ enum {
     RTCC_ENOMEM = -2,     /* device or host allocation failed */
     RTCC_ECUDA = -3,      /* a CUDA call failed; rtcc_last_cuda_error() has the cudaError_t value */
     RTCC_ENOCONV = -4,    /* micro-iterations reached max_micro; propagation state NOT advanced */
-    RTCC_ENONFINITE = -5  /* NaN/Inf met in the amplitude update; propagation state NOT advanced */
+    RTCC_ENONFINITE = -5, /* NaN/Inf met in the amplitude update; propagation state NOT advanced */
+    RTCC_EIO = -6         /* checkpoint file could not be opened / read / written, or is not a checkpoint */
 };
 
 enum { RTCC_HOST_PTRS = 1u };
@@ -84,6 +85,16 @@ int rtcc_residual_energy(const rtcc_ctx* ctx, double out[2]);
 /* Restart support: set amplitudes, time and cumulant, re-evaluate R and E there. c is a HOST pointer. */
 int rtcc_set_amplitudes(rtcc_ctx* ctx, const double* t1, const double* t2, double time, const double c[2]);
 int rtcc_get_amplitudes(const rtcc_ctx* ctx, double* t1, double* t2);
+
+/* Checkpoint / restart ("amplitudes of steps i-1 and i, Fock matrix, Cholesky vectors"): Eq. 9 is a one-step
+ * method, so the propagation state is T(tau), R(T(tau)), tau, C(tau), E(tau) and the solver settings; the Fock matrix and the
+ * Cholesky vectors are the caller's inputs to rtcc_create and are not duplicated.  rtcc_save writes them to `path` (host file
+ * system; little-endian: a 104-byte header -- magic "RTCCCKP1", o_alpha, o_beta, v_alpha, v_beta, n_chol, solver mode,
+ * max_micro, fixed_micro as int32, n_t1, n_t2 as int64, tol, tau, Re C, Im C, Re E, Im E as float64 -- then t1|t2 and r1|r2 as
+ * packed interleaved complex128).  rtcc_load restores them into a context created for the same problem (RTCC_EINVAL if the
+ * sizes differ, RTCC_EIO for a short or foreign file; the state is untouched on error).  A loaded run continues bit-identically. */
+int rtcc_save(const rtcc_ctx* ctx, const char* path);
+int rtcc_load(rtcc_ctx* ctx, const char* path);
 
 /* Solver of the implicit Eq. 9.  mode 0: plain fixed point t(k+1) = B + (i dt/2) R(t(k));
  * mode 1: orbital-energy-denominator preconditioned iteration with the same fixed point.

@@ -707,6 +707,7 @@ const char* rtcc_strerror(int code)
         case RTCC_ECUDA: return "CUDA error";
         case RTCC_ENOCONV: return "micro-iterations did not converge";
         case RTCC_ENONFINITE: return "non-finite amplitudes";
+        case RTCC_EIO: return "checkpoint file: I/O error or wrong format";
         default: return "unknown error";
     }
 }
@@ -1109,6 +1110,83 @@ int rtcc_get_amplitudes(const rtcc_ctx* c, double* t1, double* t2)
     if (copy_out(c, t1, c->t_cur, 2 * d.n_t1)) return RTCC_ECUDA;
     if (copy_out(c, t2, c->t_cur + 2 * d.n_t1, 2 * d.n_t2)) return RTCC_ECUDA;
     if (cudaStreamSynchronize(c->st) != cudaSuccess) return RTCC_ECUDA;
+    return RTCC_OK;
+}
+
+// ---- checkpoint / restart.  File: header, then t(tau) and R(t(tau)) as packed interleaved complex128.
+namespace {
+struct CkptHeader {
+    char magic[8];                 // "RTCCCKP1"
+    int oa, ob, va, vb, nchol, mode, max_micro, fixed_micro;
+    long long n_t1, n_t2;
+    double tol, time, C[2], E[2];
+};
+int stream_file(rtcc_ctx* c, FILE* f, double* dev, long long ndoubles, bool write)
+{
+    const long long chunk = 1LL << 23;                          // 64 MiB of doubles per hop through pinned memory
+    double* h = nullptr;
+    if (cudaMallocHost((void**)&h, (size_t)chunk * 8) != cudaSuccess) { cudaGetLastError(); return RTCC_ENOMEM; }
+    int rc = RTCC_OK;
+    for (long long o = 0; o < ndoubles && !rc; o += chunk) {
+        const long long m = ndoubles - o < chunk ? ndoubles - o : chunk;
+        if (write) {
+            if (cudaMemcpyAsync(h, dev + o, (size_t)m * 8, cudaMemcpyDeviceToHost, c->st) != cudaSuccess || cudaStreamSynchronize(c->st) != cudaSuccess) rc = RTCC_ECUDA;
+            else if (fwrite(h, 8, (size_t)m, f) != (size_t)m) rc = RTCC_EIO;
+        } else {
+            if (fread(h, 8, (size_t)m, f) != (size_t)m) rc = RTCC_EIO;
+            else if (cudaMemcpyAsync(dev + o, h, (size_t)m * 8, cudaMemcpyHostToDevice, c->st) != cudaSuccess || cudaStreamSynchronize(c->st) != cudaSuccess) rc = RTCC_ECUDA;
+        }
+    }
+    cudaFreeHost(h);
+    return rc;
+}
+}  // namespace
+
+int rtcc_save(const rtcc_ctx* cc, const char* path)
+{
+    rtcc_ctx* c = const_cast<rtcc_ctx*>(cc);
+    if (!c || !path) return RTCC_EINVAL;
+    FILE* f = fopen(path, "wb");
+    if (!f) return RTCC_EIO;
+    CkptHeader h;
+    memset(&h, 0, sizeof(h));
+    memcpy(h.magic, "RTCCCKP1", 8);
+    const Dims& d = c->d;
+    h.oa = d.o[0]; h.ob = d.o[1]; h.va = d.v[0]; h.vb = d.v[1]; h.nchol = d.NQ;
+    h.mode = c->mode; h.max_micro = c->max_micro; h.fixed_micro = c->fixed_micro; h.tol = c->tol;
+    h.n_t1 = d.n_t1; h.n_t2 = d.n_t2; h.time = c->time;
+    h.C[0] = c->C[0]; h.C[1] = c->C[1]; h.E[0] = c->E[0]; h.E[1] = c->E[1];
+    int rc = fwrite(&h, sizeof(h), 1, f) == 1 ? RTCC_OK : RTCC_EIO;
+    if (!rc) rc = stream_file(c, f, c->t_cur, 2 * c->namp, true);
+    if (!rc) rc = stream_file(c, f, c->r_cur, 2 * c->namp, true);
+    if (fclose(f) != 0 && !rc) rc = RTCC_EIO;
+    return rc;
+}
+
+int rtcc_load(rtcc_ctx* c, const char* path)
+{
+    if (!c || !path) return RTCC_EINVAL;
+    FILE* f = fopen(path, "rb");
+    if (!f) return RTCC_EIO;
+    CkptHeader h;
+    const Dims& d = c->d;
+    int rc = RTCC_OK;
+    if (fread(&h, sizeof(h), 1, f) != 1 || memcmp(h.magic, "RTCCCKP1", 8) != 0) rc = RTCC_EIO;
+    else if (h.oa != d.o[0] || h.ob != d.o[1] || h.va != d.v[0] || h.vb != d.v[1] || h.nchol != d.NQ || h.n_t1 != d.n_t1 || h.n_t2 != d.n_t2)
+        rc = RTCC_EINVAL;                          // written for another problem
+    if (!rc) {
+        // read into the iterate buffers first so that a short file leaves the propagation state untouched
+        rc = stream_file(c, f, c->gx, 2 * c->namp, false);
+        if (!rc) rc = stream_file(c, f, c->gr, 2 * c->namp, false);
+        if (!rc && fgetc(f) != EOF) rc = RTCC_EIO;
+    }
+    fclose(f);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->t_cur, c->gx, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    c->mode = h.mode; c->max_micro = h.max_micro; c->fixed_micro = h.fixed_micro; c->tol = h.tol;
+    c->time = h.time; c->C[0] = h.C[0]; c->C[1] = h.C[1]; c->E[0] = h.E[0]; c->E[1] = h.E[1];
     return RTCC_OK;
 }
 

@@ -22,7 +22,7 @@ SYMBOLS = [
     "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
     "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
-    "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy",
+    "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy", "rtcc_save", "rtcc_load",
 ]
 
 
@@ -65,6 +65,8 @@ def load():
         lib.rtcc_set_default_option.argtypes = [ctypes.c_char_p, i]
         lib.rtcc_ladder_plan.argtypes = [vp, i, P(i)]
         lib.rtcc_ladder_occupancy.argtypes = [vp, P(i)]
+        lib.rtcc_save.argtypes = [vp, ctypes.c_char_p]
+        lib.rtcc_load.argtypes = [vp, ctypes.c_char_p]
         lib.rtcc_last_cuda_error.argtypes = [vp]
         lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
         _lib = lib
@@ -227,6 +229,13 @@ class Rtcc:
         t1, t2 = self._new(self.n_t1), self._new(self.n_t2)
         self._ck(self._lib.rtcc_get_amplitudes(self._h, _ptr(t1), _ptr(t2)), "rtcc_get_amplitudes")
         return t1, t2
+
+    def save(self, path: str):
+        """Checkpoint T(tau), R(T(tau)), tau, C, E and the solver settings."""
+        self._ck(self._lib.rtcc_save(self._h, os.fsencode(path)), "rtcc_save")
+
+    def load(self, path: str):
+        self._ck(self._lib.rtcc_load(self._h, os.fsencode(path)), "rtcc_load")
 
     def set_solver(self, mode=0, tol=1e-4, max_micro=200, fixed_micro=0):
         self._ck(self._lib.rtcc_set_solver(self._h, mode, tol, max_micro, fixed_micro), "rtcc_set_solver")

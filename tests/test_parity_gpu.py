@@ -295,6 +295,54 @@ def test_step_errors_leave_state_untouched(rtcc):
     other.close()
 
 
+def test_checkpoint_restart_continues_bit_identically_and_matches_oracle(rtcc, tmp_path):
+    """NEXT-4: run, rtcc_save, destroy, create, rtcc_load, continue.  The restarted run must equal the
+    uninterrupted library run bit for bit AND the oracle propagated straight through within the 1e-8 tolerance on C."""
+    cfg = inputs.CONFIGS["tiny"]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=0.2)
+    prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+    po = orc.Propagator(prob, mode=1, tol=1e-12, max_micro=200)
+    straight = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)
+    straight.set_solver(mode=1, tol=1e-12, max_micro=200)
+    first = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)
+    first.set_solver(mode=1, tol=1e-12, max_micro=200)
+    path = str(tmp_path / "ckpt.bin")
+    for _ in range(7):
+        po.step(cfg.dt); straight.step(cfg.dt); first.step(cfg.dt)
+    first.save(path)
+    first.close()
+    import os
+    assert os.path.getsize(path) == 104 + 2 * 16 * (straight.n_t1 + straight.n_t2)
+    second = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)          # default solver settings: the file restores mode / tol / limits
+    second.load(path)
+    assert second.time == straight.time and second.cumulant() == straight.cumulant()
+    for _ in range(6):
+        po.step(cfg.dt); straight.step(cfg.dt); second.step(cfg.dt)
+    assert second.cumulant() == straight.cumulant() and second.time == straight.time
+    a, b = second.get_amplitudes(), straight.get_amplitudes()
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    C, E = second.cumulant()
+    assert abs(C - po.C) <= CTOL * abs(po.C) and abs(E - po.E) <= CTOL * abs(po.E)
+    # a foreign / truncated file and a checkpoint of another problem are refused and leave the state alone
+    bad = str(tmp_path / "bad.bin")
+    open(bad, "wb").write(b"not a checkpoint")
+    with pytest.raises(rtcc.RtccError) as ei:
+        second.load(bad)
+    assert ei.value.code == -6
+    data = open(path, "rb").read()
+    open(bad, "wb").write(data[: len(data) // 2])
+    with pytest.raises(rtcc.RtccError) as ei:
+        second.load(bad)
+    assert ei.value.code == -6 and second.cumulant() == straight.cumulant()
+    L2, f2 = rand_problem(2, 3, 4, 3, 5, seed=1)
+    other = rtcc.Rtcc(2, 3, 4, 3, 5, L2, f2)
+    with pytest.raises(rtcc.RtccError) as ei:
+        other.load(path)
+    assert ei.value.code == -1
+    for c in (straight, second, other):
+        c.close()
+
+
 def test_contraction_primitive_against_matmul(rtcc):
     rng = np.random.default_rng(0)
     # the last shape is large enough (two full waves of 128x128 tiles) to run the big-tile kernel
