@@ -170,8 +170,9 @@ __global__ void k_add_Lvo(Dims d, const double* __restrict__ Lt0, const double* 
 
 // W[(m,e)][pl][(j,b)] += -1/2 delta_mj Fvv[b][e] + 1/2 delta_be Foo[m][j]
 // (Fvv / Foo are the vv / oo blocks of the two dressed-Fock buffers; rows are (m of spin so, e of spin sv))
+// Only columns with j in [jlo, jhi) are touched (a column slab of W holds those j; coff is then relative to the slab).
 __global__ void k_add_Fd(int om, int ve, int n, const double* __restrict__ Fo, int oo_, const double* __restrict__ Fv, int ov_,
-                         double* __restrict__ W, long long ldW, long long poff, long long roff, long long coff)
+                         double* __restrict__ W, long long ldW, long long poff, long long roff, long long coff, int jlo, int jhi)
 {
     // Fo: dressed Fock of the occupied index' spin (planar [2][n][n]), oo_ = its o; Fv likewise for the virtual index
     const long long nn = (long long)n * n;
@@ -181,6 +182,7 @@ __global__ void k_add_Fd(int om, int ve, int n, const double* __restrict__ Fo, i
             if (x < tot1) {          // (m, e, b): j = m
                 int m = (int)(x / ((long long)ve * ve)); int r = (int)(x - (long long)m * ve * ve);
                 int e = r / ve, b = r - e * ve;
+                if (m < jlo || m >= jhi) continue;
                 double f = Fv[pl * nn + (long long)(ov_ + b) * n + ov_ + e];
                 // b == e also gets the Foo[m][m] piece here so that each W element is touched by one thread only
                 double add = -0.5 * f;
@@ -190,7 +192,7 @@ __global__ void k_add_Fd(int om, int ve, int n, const double* __restrict__ Fo, i
                 long long y = x - tot1;
                 int m = (int)(y / ((long long)om * ve)); int r = (int)(y - (long long)m * om * ve);
                 int j = r / ve, e = r - j * ve;
-                if (j == m) continue;
+                if (j == m || j < jlo || j >= jhi) continue;
                 double f = Fo[pl * nn + (long long)m * n + j];
                 W[(roff + (long long)m * ve + e) * ldW + pl * poff + coff + (long long)j * ve + e] += 0.5 * f;
             }
@@ -270,6 +272,190 @@ __global__ void k_assemble(Dims d, AsmArgs A)
             }
         }
         A.r2p[2 * x] = out[0]; A.r2p[2 * x + 1] = out[1];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Low-memory ("lean") pipeline: BASELINE.json config 5 does not fit 180 GB with the pair-space matrices held whole
+// (Table 2: the paper's storage argument is three amplitude-sized tensors plus the Cholesky
+// vectors).  There the same-spin pair-space blocks are the only unpacked amplitudes, the alpha-beta block is read in place
+// from the packed boundary layout through strides, the ring intermediates W and Z live in column slabs that are folded
+// into the packed residual slab by slab, and the ladder's buffers reuse the memory of the ring phase.
+
+// Tss[(i,a)][pl][(m,e)] = t_{im}^{ae} for one spin (planar, n1s x 2 n1s)
+__global__ void k_build_Tss(Dims d, int s, const double* __restrict__ t2p, double* __restrict__ T)
+{
+    const int v = d.v[s];
+    const long long n1s = (long long)d.o[s] * v, tot = n1s * n1s;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        const long long r = x / n1s, c = x - r * n1s;
+        const int i = (int)(r / v), a = (int)(r - (long long)i * v), m = (int)(c / v), e = (int)(c - (long long)m * v);
+        c128 z = ss_amp(t2p, d.off_t2[s], d.pv[s], i, m, a, e);
+        T[r * 2 * n1s + c] = z.re;
+        T[r * 2 * n1s + n1s + c] = z.im;
+    }
+}
+
+// tile-major ladder amplitudes only (no planar copy, no tau): alpha-beta and same-spin
+__global__ void k_build_Xt_ab(Dims d, const double* __restrict__ t2p, double* __restrict__ Xt, int nFt, int ncol, int nt2)
+{
+    const long long tot = (long long)d.v[0] * d.v[1] * d.oo;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        // x runs over the packed order (i, J, e, F) so that the reads are contiguous
+        const long long vv = (long long)d.v[0] * d.v[1];
+        const int col = (int)(x / vv); const long long ef = x - (long long)col * vv;
+        const int e = (int)(ef / d.v[1]), F = (int)(ef - (long long)e * d.v[1]);
+        const long long k = d.off_t2[2] + x;
+        Xt[xt_index(e, F, col, nFt, ncol, nt2)] = t2p[2 * k];
+        Xt[xt_index(e, F, d.oo + col, nFt, ncol, nt2)] = t2p[2 * k + 1];
+    }
+}
+__global__ void k_build_Xt_ss(Dims d, int s, const double* __restrict__ t2p, const int2* __restrict__ opairs, double* __restrict__ Xt, int nFt, int ncol, int nt2)
+{
+    const int v = d.v[s], po = d.po[s];
+    const long long tot = (long long)v * v * po;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        const long long row = x / po; const int col = (int)(x - row * po);
+        const int e = (int)(row / v), f = (int)(row - (long long)e * v);
+        const int2 ij = opairs[col];
+        c128 z = ss_amp(t2p, d.off_t2[s], d.pv[s], ij.x, ij.y, e, f);
+        Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
+        Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;
+    }
+}
+
+// V[(m,N)][pl][(i,J)] = Woo[(m,N)][pl][(i,J)] + Y[(m, N) row of the all-orbital ladder output][pl][(i,J)]   (alpha-beta o^4 pieces)
+__global__ void k_add_oo_rows(int oa, int ob, int n, long long oo, const double* __restrict__ Woo, const double* __restrict__ Y, double* __restrict__ V)
+{
+    const long long tot = oo * 2 * oo;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        const long long r = x / (2 * oo), c = x - r * 2 * oo;
+        const int m = (int)(r / ob), N = (int)(r - (long long)m * ob);
+        V[x] = Woo[x] + Y[((long long)m * n + N) * 2 * oo + c];
+    }
+}
+// same spin: Vp[(m<n)][pl][(i<j)] = W4 antisymmetrised + Y rows (m,n);  Yoo[(m,n)][pl][(i<j)] = antisymmetric unpacking of the Y rows (m<n)
+__global__ void k_ss_prep_lean(int o, int po, int n, const int2* __restrict__ opairs, const double* __restrict__ W4,
+                               const double* __restrict__ Y, double* __restrict__ Vp, double* __restrict__ Yoo)
+{
+    const long long tot = (long long)po * po;
+    const int o2 = o * o;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        const int r = (int)(x / po), c = (int)(x - (long long)r * po);
+        const int2 mn = opairs[r], ij = opairs[c];
+        const long long row = (long long)(mn.x * o + mn.y) * 2 * o2;
+        for (int pl = 0; pl < 2; ++pl) {
+            const double y = Y[((long long)mn.x * n + mn.y) * 2 * po + pl * po + c];
+            Vp[(long long)r * 2 * po + pl * po + c] = W4[row + pl * o2 + ij.x * o + ij.y] - W4[row + pl * o2 + ij.y * o + ij.x] + y;
+            Yoo[((long long)mn.x * o + mn.y) * 2 * po + pl * po + c] = y;
+            Yoo[((long long)mn.y * o + mn.x) * 2 * po + pl * po + c] = -y;
+        }
+    }
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < (long long)o * 2 * po; x += (long long)gridDim.x * blockDim.x) {
+        const int m = (int)(x / (2 * po)); const long long c = x - (long long)m * 2 * po;
+        Yoo[((long long)m * o + m) * 2 * po + c] = 0.0;
+    }
+}
+// offsets of the ladder-output rows (o+a, o+b), a < b, by packed virtual pair index
+__global__ void k_pair_row_table(int o, int n, int pv, long long ld, const int2* __restrict__ vpairs, long long* __restrict__ tab)
+{
+    for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < pv; x += gridDim.x * blockDim.x) {
+        const int2 ab = vpairs[x];
+        tab[x] = ((long long)(o + ab.x) * n + o + ab.y) * ld;
+    }
+}
+
+// Fold one slab of a ring intermediate into the packed residual:  r2 (+)= signed sum of the slab's elements each packed
+// element depends on.  kind 0/1: columns (j,b) of spin kind with j in [j0, j1) of Z_sc (rows: all n1 pairs);
+// kind 2: Z_AB[(i,B),(J,a)] whole, kind 3: Z_BA[(J,a),(i,B)] whole (both subtracted from the alpha-beta block).
+// Z is planar with row pitch 2*wc (wc = columns held).  Every packed element is owned by one thread: no atomics.
+__global__ void k_fold_slab(Dims d, int kind, int j0, int j1, const double* __restrict__ Z, long long wc,
+                            const int2* __restrict__ op, const int2* __restrict__ vp, double* __restrict__ r2p)
+{
+    const long long nss0 = (long long)d.po[0] * d.pv[0], nss1 = (long long)d.po[1] * d.pv[1];
+    const long long nab = (long long)d.oo * d.v[0] * d.v[1];
+    const long long ld = 2 * wc;
+    if (kind <= 1) {
+        const int s = kind, v = d.v[s];
+        const long long rbase = s ? d.n1a : 0;          // row offset of spin-s pairs in the n1 rows
+        const long long c0 = (long long)j0 * v;
+        // same-spin block of spin s: Z[ia,jb] - Z[ja,ib] - Z[ib,ja] + Z[jb,ia]
+        const long long nss = s ? nss1 : nss0, off = s ? nss0 : 0;
+        for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < nss; x += (long long)gridDim.x * blockDim.x) {
+            const int pij = (int)(x / d.pv[s]), pab = (int)(x - (long long)pij * d.pv[s]);
+            const int2 ij = op[pij], ab = vp[pab];
+            double re = 0.0, im = 0.0;
+            bool any = false;
+            // terms (row occupied, row virtual, column occupied, column virtual, sign)
+            const int t[4][5] = {{ij.x, ab.x, ij.y, ab.y, 1}, {ij.y, ab.x, ij.x, ab.y, -1}, {ij.x, ab.y, ij.y, ab.x, -1}, {ij.y, ab.y, ij.x, ab.x, 1}};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (t[k][2] >= j0 && t[k][2] < j1) {
+                    const long long row = rbase + (long long)t[k][0] * v + t[k][1], col = (long long)t[k][2] * v + t[k][3] - c0;
+                    re += t[k][4] * Z[row * ld + col]; im += t[k][4] * Z[row * ld + wc + col];
+                    any = true;
+                }
+            }
+            if (any) { r2p[2 * (off + x)] += re; r2p[2 * (off + x) + 1] += im; }
+        }
+        // alpha-beta block: Z[ia,JB] (column beta) or Z[JB,ia] (column alpha)
+        for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < nab; x += (long long)gridDim.x * blockDim.x) {
+            long long k = x;
+            const int B = (int)(k % d.v[1]); k /= d.v[1];
+            const int a = (int)(k % d.v[0]); k /= d.v[0];
+            const int J = (int)(k % d.o[1]); const int i = (int)(k / d.o[1]);
+            long long row, col; int jc;
+            if (s == 1) { row = (long long)i * d.v[0] + a; col = (long long)J * d.v[1] + B; jc = J; }
+            else { row = d.n1a + (long long)J * d.v[1] + B; col = (long long)i * d.v[0] + a; jc = i; }
+            if (jc < j0 || jc >= j1) continue;
+            col -= c0;
+            r2p[2 * (nss0 + nss1 + x)] += Z[row * ld + col];
+            r2p[2 * (nss0 + nss1 + x) + 1] += Z[row * ld + wc + col];
+        }
+    } else {
+        for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < nab; x += (long long)gridDim.x * blockDim.x) {
+            long long k = x;
+            const int B = (int)(k % d.v[1]); k /= d.v[1];
+            const int a = (int)(k % d.v[0]); k /= d.v[0];
+            const int J = (int)(k % d.o[1]); const int i = (int)(k / d.o[1]);
+            const long long iB = (long long)i * d.v[1] + B, Ja = (long long)J * d.v[0] + a;
+            const long long row = kind == 2 ? iB : Ja, col = kind == 2 ? Ja : iB;
+            r2p[2 * (nss0 + nss1 + x)] -= Z[row * ld + col];
+            r2p[2 * (nss0 + nss1 + x) + 1] -= Z[row * ld + wc + col];
+        }
+    }
+}
+
+// last pass of the lean assembly: r2 += ladder pieces (the T1 and o^4 corrections are already inside Y), r1 = r1buf + f~_ai
+__global__ void k_fold_ladder(Dims d, AsmArgs A)
+{
+    const long long nss0 = (long long)d.po[0] * d.pv[0], nss1 = (long long)d.po[1] * d.pv[1];
+    const long long tot = d.n_t2 + d.n_t1;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        if (x >= d.n_t2) {
+            const long long k = x - d.n_t2;
+            const int s = k >= d.n1a; const int cc = (int)(s ? k - d.n1a : k);
+            const int i = cc / d.v[s], a = cc - i * d.v[s];
+            const long long nn = (long long)d.n * d.n;
+            for (int pl = 0; pl < 2; ++pl)
+                A.r1p[2 * k + pl] = A.r1buf[pl * (long long)d.n1 + k] + A.Ft[s][pl * nn + (long long)(d.o[s] + a) * d.n + i];
+            continue;
+        }
+        if (x < nss0 + nss1) {
+            const int s = x >= nss0; const long long k = s ? x - nss0 : x;
+            const int pij = (int)(k / d.pv[s]), pab = (int)(k - (long long)pij * d.pv[s]);
+            const int2 ab = A.vpairs[s][pab];
+            const int po = d.po[s], o = d.o[s];
+            for (int pl = 0; pl < 2; ++pl)
+                A.r2p[2 * x + pl] += A.Yss[s][((long long)(o + ab.x) * d.n + o + ab.y) * 2 * po + pl * po + pij];
+        } else {
+            long long k = x - nss0 - nss1;
+            const int B = (int)(k % d.v[1]); k /= d.v[1];
+            const int a = (int)(k % d.v[0]); k /= d.v[0];
+            const int J = (int)(k % d.o[1]); const int i = (int)(k / d.o[1]);
+            for (int pl = 0; pl < 2; ++pl)
+                A.r2p[2 * x + pl] += A.Yab[((long long)(d.o[0] + a) * d.n + d.o[1] + B) * 2 * d.oo + pl * d.oo + i * d.o[1] + J];
+        }
     }
 }
 

@@ -699,16 +699,10 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const Ladder
         if (!first) continue;
         long long clusters = 0;
         for (int k = i; k < b.ncase; ++k) if (b.c[k].cl == g.cl) clusters += (long long)b.c[k].ntiles * b.c[k].ngrp;
-        const int conc = occ.act[g.cl] / g.cl > 0 ? occ.act[g.cl] / g.cl : 1;
+        // wide launches are not sliced on their own: every slice needs a partial output buffer the size of Y (GBs at the
+        // sizes that run here) for a gain of a few per cent in wave quantisation
+        (void)clusters;
         int S = 1;
-        if (clusters < 8LL * conc) {
-            double beff = 0.0;
-            for (int T = 1; T <= max_split; ++T) {
-                double w = (double)clusters * T / conc;
-                double eff = w / ceil(w);
-                if (eff > beff + 0.02) { beff = eff; S = T; }
-            }
-        }
         if (tune.force_split >= 1) S = tune.force_split;
         int it = 0;
         for (int k = i; k < b.ncase; ++k) {

@@ -20,6 +20,7 @@ using namespace rtcc;
 // process-wide defaults read by rtcc_create (rtcc_set_default_option, include/rtcc.h)
 struct RtccOptions {
     int fused = 1, fused_fock = 1, graph = 1, prio = 1, tile = 0;
+    int lean = -1, lean_slab_j = 0;              // lean: -1 automatic (when the standard layout does not fit), 0 never, 1 always
     LadderTune lad;
 };
 static RtccOptions g_opt;
@@ -50,6 +51,14 @@ struct rtcc_ctx {
     double *Xss[2]{}, *tauss[2]{}, *Yss[2]{}, *W4[2]{}, *Wp[2]{}, *Yoop[2]{}, *Zv[2]{};
     int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
     int ntiles_ab = 0, ntiles_ss[2]{};
+    // low-memory pipeline: one arena reused by the ring phase and the ladder phase
+    bool lean = false;
+    double* arena = nullptr; long long arena_cap = 0;
+    double *Tss[2]{}, *Wslab = nullptr, *Zslab = nullptr, *Wsf = nullptr, *Zsf = nullptr;
+    int slab_j[2]{1, 1};                                         // occupied indices j per column slab, by spin
+    double *Voo = nullptr, *Vp[2]{}, *Yoo[2]{};
+    long long* cmp[2]{};                                         // ladder-output row offsets by packed virtual pair
+    long long xt_ab_cnt = 0, xt_ss_cnt[2]{};
     LadderBatch lb{};
     LadderOcc locc{};
     RtccOptions opt{};
@@ -426,7 +435,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             run(c, g);
         }
         if (s == 0 || d.n1a == 0) { WAITEV(1, 2); WAITEV(1, 7); }
-        EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1);
+        EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1, 0, o);
     }
     LINK(1, 0, 3);
     BR(0);
@@ -467,7 +476,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         }
         WAITEV(2, 2);
         WAITEV(2, 7);
-        EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL);
+        EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL, 0, ob);
         {
             TcGemm g = G0(nA, nB, nB);
             setA(g, 0, lB, 0, 0, 1, 0, 1);
@@ -495,7 +504,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             g.beta = 1.0;
             run(c, g);
         }
-        EW(c, k_add_Fd, (long long)oa * vb * vb + (long long)oa * oa * vb, oa, vb, n, c->Ft[0], oa, c->Ft[1], ob, c->WAA, lA, (long long)nA, 0LL, 0LL);
+        EW(c, k_add_Fd, (long long)oa * vb * vb + (long long)oa * oa * vb, oa, vb, n, c->Ft[0], oa, c->Ft[1], ob, c->WAA, lA, (long long)nA, 0LL, 0LL, 0, oa);
         {
             TcGemm g = G0(nB, nA, nA);
             setA(g, 0, 1, 0, 0, lB, 0, 0);
@@ -650,6 +659,550 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
 
 namespace {
 
+// ---------------------------------------------------------------------------------------------
+// Low-memory evaluation of the same working equations (DESIGN.md sections 4 and 5).  Differences from residual_pipeline:
+// one stream (the phases reuse one arena); the alpha-beta amplitudes are read in place from the packed input through
+// two-level strides (interleaved complex: plane offset 1); the same-spin pair-space blocks are the only unpacked
+// amplitudes; W and Z of the spin-conserving ring sector live in column slabs (a range of occupied indices j of one spin)
+// that k_fold_slab adds into the packed residual; the spin-flip sector reuses the same memory; the ladder's buffers
+// overlay the ring phase's; tau is never formed (tau = t + t1 t1 is applied as two contractions) and the T1 corrections
+// are accumulated into the ladder output instead of a separate buffer.
+// ---------------------------------------------------------------------------------------------
+struct TOp { const double* p; long long pim, r_hi, r_lo, c_hi, c_lo; int Rlo, Clo; };
+
+// T[(row pair of spin sr), (column pair of spin sc)] = t_{im}^{ae} as a strided operand (strides in doubles)
+TOp t_block(const rtcc_ctx* c, const double* x, int sr, int sc)
+{
+    const Dims& d = c->d;
+    TOp t{};
+    if (sr == sc) {
+        const long long n1s = (long long)d.o[sr] * d.v[sr];
+        t.p = c->Tss[sr]; t.pim = n1s; t.r_hi = 0; t.r_lo = 2 * n1s; t.Rlo = 0; t.c_hi = 0; t.c_lo = 1; t.Clo = 0;
+    } else {
+        const long long va = d.v[0], vb = d.v[1], ob = d.o[1];
+        t.p = x + 2 * d.n_t1 + 2 * d.off_t2[2]; t.pim = 1;
+        if (sr == 0) { t.Rlo = (int)va; t.r_hi = 2 * ob * va * vb; t.r_lo = 2 * vb; t.Clo = (int)vb; t.c_hi = 2 * va * vb; t.c_lo = 2; }
+        else         { t.Rlo = (int)vb; t.r_hi = 2 * va * vb; t.r_lo = 2; t.Clo = (int)va; t.c_hi = 2 * ob * va * vb; t.c_lo = 2 * vb; }
+    }
+    return t;
+}
+
+int residual_pipeline_lean(rtcc_ctx* c, const double* x, double* r)
+{
+    const Dims& d = c->d;
+    const int n = d.n, NQ = d.NQ, n1 = d.n1;
+    const long long nn = (long long)n * n, plane = (long long)NQ * nn, ld1 = 2LL * n1;
+    const double* t1p = x;
+    const double* t2p = x + 2 * d.n_t1;
+    for (int i = 0; i < 8; ++i) c->S[i] = c->st;
+    c->si = 0;
+#define STL (c->st)
+    const long long rowoff[2] = {0, d.n1a};
+    const long long n1s_[2] = {d.n1a, d.n1b};
+
+    // ---- 1. t1 planar; same-spin pair-space blocks; residual accumulator cleared
+    c->sec = 1;
+    EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
+    for (int s = 0; s < 2; ++s)
+        if (n1s_[s] > 0) EW(c, k_build_Tss, n1s_[s] * n1s_[s], d, s, t2p, c->Tss[s]);
+    CK(cudaMemsetAsync(r, 0, (size_t)c->namp * 16, STL));
+
+    // ---- 2. T1-dressed Cholesky vectors (general path) and gamma
+    c->sec = 2;
+    if (c->fused_dress) {
+        DressArgs da;
+        for (int s = 0; s < 2; ++s) { da.L[s] = c->L[s]; da.Lt[s] = c->Lt[s]; }
+        da.t1r = c->t1r; da.gam = c->gam;
+        k_dress<<<NQ, 256, dress_smem(d), STL>>>(d, da);
+        c->launches++;
+    } else {
+        for (int s = 0; s < 2; ++s) {
+            const int o = d.o[s], v = d.v[s];
+            const long long off1 = rowoff[s];
+            CK(cudaMemcpyAsync(c->Lt[s], c->L[s], plane * 8, cudaMemcpyDeviceToDevice, STL));
+            CK(cudaMemsetAsync(c->Lt[s] + plane, 0, plane * 8, STL));
+            if (o == 0) continue;
+            {
+                TcGemm g = G0(NQ * n, o, v);
+                setA(g, 0, n, 0, 0, 1, 0, 1);
+                setB(g, 0, 1, 0, v, 0, 0);
+                setC(g, 0, n, 0, 1);
+                ops_rc(g, c->L[s] + o, c->t1r + off1, n1, c->Lt[s], plane);
+                g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(v, NQ * n, o);
+                setA(g, 0, 1, 0, 0, v, 0, 0);
+                setB(g, 0, n, nn, 1, n, 1);
+                setC(g, 0, n, nn, 1);
+                ops_cc(g, c->t1r + off1, n1, c->Lt[s], plane, c->Lt[s] + (long long)o * n, plane);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+        }
+        for (int s = 0; s < 2; ++s) {
+            const int o = d.o[s], v = d.v[s];
+            TcGemm g = G0(NQ, 1, o * v);
+            setA(g, 0, nn, 0, n, 1, v, 1);
+            setB(g, v, 1, 0, 0, 0, 0);
+            setC(g, 0, 1, 0, 0);
+            ops_rc(g, c->L[s] + o, c->t1r + rowoff[s], n1, c->gam, NQ);
+            g.beta = s ? 1.0 : 0.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 4. M^Q_(col) = sum_(me) L^Q_me T[(me),(col)]: per column spin, the same-spin block then the alpha-beta block
+    c->sec = 4;
+    for (int sc = 0; sc < 2; ++sc) {
+        if (n1s_[sc] == 0) continue;
+        bool first = true;
+        for (int k = 0; k < 2; ++k) {
+            const int sr = k == 0 ? sc : 1 - sc;
+            const int o = d.o[sr], v = d.v[sr];
+            if (n1s_[sr] == 0) continue;
+            const TOp t = t_block(c, x, sr, sc);
+            if (sr == sc) {          // planar block: one real GEMM over the stacked Re|Im columns
+                TcGemm g = G0(NQ, 2 * (int)n1s_[sc], o * v);
+                setA(g, 0, nn, 0, n, 1, v, 1);
+                setB(g, (long long)v * t.r_lo, t.r_lo, n1s_[sc], 1, (int)n1s_[sc], 1);
+                setC(g, 0, ld1, n1, 1);
+                ops_rr(g, c->L[sr] + o, t.p, c->Mq + rowoff[sc]);
+                g.beta = first ? 0.0 : 1.0;
+                run(c, g);
+            } else {
+                TcGemm g = G0(NQ, (int)n1s_[sc], o * v);
+                setA(g, 0, nn, 0, n, 1, v, 1);
+                setB(g, t.r_hi, t.r_lo, t.c_hi, t.c_lo, t.Clo, t.c_lo < t.r_lo);
+                setC(g, 0, ld1, t.Clo, 1);                 // the column index of C is split like B's (shared Nlo)
+                ops_rc(g, c->L[sr] + o, t.p, t.pim, c->Mq + rowoff[sc], n1);
+                g.beta = first ? 0.0 : 1.0;
+                run(c, g);
+            }
+            first = false;
+        }
+    }
+
+    // ---- 5. E
+    c->sec = 5;
+    {
+        EnergyArgs ea;
+        for (int s = 0; s < 2; ++s) { ea.L[s] = c->L[s]; ea.Lt[s] = c->Lt[s]; ea.fock[s] = c->fockd[s]; }
+        ea.t1r = c->t1r; ea.Mq = c->Mq; ea.gam = c->gam; ea.partial = c->partial;
+        ea.counter = c->counters; ea.out = c->scal;
+        k_energy<<<RED_BLOCKS, RED_THREADS, 0, STL>>>(d, ea);
+        c->launches += 1;
+    }
+
+    // ---- 6. dressed Fock, F_ae, F_mi (as residual_pipeline, general path)
+    c->sec = 6;
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = rowoff[s];
+        double* F = c->Ft[s];
+        CK(cudaMemcpyAsync(F, c->Fb[s], nn * 8, cudaMemcpyDeviceToDevice, STL));
+        CK(cudaMemsetAsync(F + nn, 0, nn * 8, STL));
+        {
+            TcGemm g = G0((int)nn, 1, NQ);
+            setA(g, 0, 1, 0, 0, nn, 0, 0);
+            setB(g, 0, 1, 0, 0, 0, 0);
+            setC(g, 0, 1, 0, 0);
+            ops_rc(g, c->L[s], c->gam, NQ, F, nn);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        if (o > 0) {
+            {
+                TcGemm g = G0(n, o, v);
+                setA(g, 0, n, 0, 0, 1, 0, 1);
+                setB(g, 0, 1, 0, v, 0, 0);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, F + o, nn, c->t1r + off1, n1, F, nn);
+                g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(v, n, o);
+                setA(g, 0, 1, 0, 0, v, 0, 0);
+                setB(g, 0, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, c->t1r + off1, n1, F, nn, F + (long long)o * n, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(n, n, NQ * o);
+                setA(g, 0, n, 0, nn, 1, o, 1);
+                setB(g, nn, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cc(g, c->Lt[s], plane, c->Lt[s], plane, F, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(v, v, NQ * o);
+                setA(g, 0, 1, 0, ld1, v, o, 0);
+                setB(g, nn, n, 0, 1, 0, 1);
+                setC(g, 0, n, 0, 1);
+                ops_cr(g, c->Mq + off1, n1, c->L[s] + o, F + (long long)o * n + o, nn);
+                g.alpha = -1.0; g.beta = 1.0;
+                run(c, g);
+            }
+            {
+                TcGemm g = G0(o, o, NQ * v);
+                setA(g, 0, n, 0, nn, 1, v, 1);
+                setB(g, ld1, 1, 0, v, 0, 0);
+                setC(g, 0, n, 0, 1);
+                ops_rc(g, c->L[s] + o, c->Mq + off1, n1, F, nn);
+                g.beta = 1.0;
+                run(c, g);
+            }
+        }
+    }
+
+    // ---- 7. singles: r1 = sum_me T[(ia),(me)] f~_me (block by block) - sum_Q,n M_na L~_ni + sum_Q,f M_if L~_af
+    c->sec = 7;
+    for (int sr = 0; sr < 2; ++sr) {
+        if (n1s_[sr] == 0) continue;
+        bool first = true;
+        for (int sk = 0; sk < 2; ++sk) {
+            const int o = d.o[sk], v = d.v[sk];
+            if (n1s_[sk] == 0) continue;
+            const TOp t = t_block(c, x, sr, sk);
+            TcGemm g = G0((int)n1s_[sr], 1, o * v);
+            if (sr == sk) setA(g, 0, t.r_lo, 0, v, 1, v, 1);
+            else setA(g, t.r_hi, t.r_lo, t.Rlo, t.c_hi, t.c_lo, t.Clo, t.c_lo < t.r_lo);
+            setB(g, n, 1, 0, 0, 0, 0);
+            setC(g, sr == sk ? 0 : t.Rlo, 1, 0, 0);      // row index of C split like A's (shared Mlo)
+            ops_cc(g, t.p, t.pim, c->Ft[sk] + o, nn, c->r1buf + rowoff[sr], n1);
+            g.beta = first ? 0.0 : 1.0;
+            run(c, g);
+            first = false;
+        }
+        if (first) CK(cudaMemsetAsync(c->r1buf + rowoff[sr], 0, 0, STL));
+    }
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s];
+        const long long off1 = rowoff[s];
+        if (o == 0) continue;
+        {
+            TcGemm g = G0(o, v, NQ * o);
+            setA(g, 0, 1, 0, nn, n, o, 0);
+            setB(g, ld1, v, 0, 1, 0, 1);
+            setC(g, 0, v, 0, 1);
+            ops_cc(g, c->Lt[s], plane, c->Mq + off1, n1, c->r1buf + off1, n1);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(o, v, NQ * v);
+            setA(g, 0, v, 0, ld1, 1, v, 1);
+            setB(g, nn, 1, 0, n, 0, 0);
+            setC(g, 0, v, 0, 1);
+            ops_cc(g, c->Mq + off1, n1, c->Lt[s] + (long long)o * n + o, plane, c->r1buf + off1, n1);
+            g.beta = 1.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 8. N^Q_ia = L~^Q_ai + M^Q_ia; o^4 integrals <mn||ij>~ (the dressed vectors are dead once the ring is done)
+    c->sec = 8;
+    EW(c, k_add_Lvo, (long long)NQ * 2 * n1, d, c->Lt[0], c->Lt[1], c->Mq, c->Nq);
+    if (d.oo > 0) {
+        const int oa = d.o[0], ob = d.o[1];
+        const long long lY = 2LL * d.oo;
+        TcGemm g = G0(oa * oa, ob * ob, NQ);
+        setA(g, n, 1, oa, 0, nn, 0, 0);
+        setB(g, 0, nn, n, 1, ob, 1);
+        setC(g, ob * lY, ob, lY, 1);
+        ops_cc(g, c->Lt[0], plane, c->Lt[1], plane, c->Wooab, d.oo);
+        run(c, g);
+    }
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s];
+        if (d.po[s] == 0) continue;
+        const long long o2 = (long long)o * o;
+        TcGemm g = G0(o * o, o * o, NQ);
+        setA(g, n, 1, o, 0, nn, 0, 0);
+        setB(g, 0, nn, n, 1, o, 1);
+        setC(g, o * 2 * o2, o, 2 * o2, 1);
+        ops_cc(g, c->Lt[s], plane, c->Lt[s], plane, c->W4[s], o2);
+        run(c, g);
+    }
+
+    // ---- 9. spin-conserving ring sector, one column slab (occupied indices j0..j1 of spin sc) at a time:
+    //         W[:, slab] = 1/2 Kx T[:, slab] + Xd + Fd ;   Z[:, slab] = 1/2 N^T N[:, slab] - T W[:, slab] ;   r2 += fold(Z slab)
+    c->sec = 9;
+    for (int sc = 0; sc < 2; ++sc) {
+        const int osc = d.o[sc], vsc = d.v[sc];
+        if (n1s_[sc] == 0) continue;
+        for (int j0 = 0; j0 < osc; j0 += c->slab_j[sc]) {
+            const int j1 = j0 + c->slab_j[sc] < osc ? j0 + c->slab_j[sc] : osc;
+            const long long wc = (long long)(j1 - j0) * vsc, ldW = 2 * wc, c0 = (long long)j0 * vsc;
+            for (int sr = 0; sr < 2; ++sr) {
+                const int o = d.o[sr], v = d.v[sr];
+                if (n1s_[sr] == 0) continue;
+                const TOp t = t_block(c, x, sr, sc);
+                double* Wr = c->Wslab + rowoff[sr] * ldW;
+                if (sr == sc) {
+                    TcGemm g = G0((int)n1s_[sr], (int)(2 * wc), (int)n1s_[sr]);
+                    setA(g, 0, n1s_[sr], 0, 0, 1, 0, 1);
+                    setB(g, 0, t.r_lo, n1s_[sc], 1, (int)wc, 1);
+                    setC(g, 0, ldW, wc, 1);
+                    ops_rr(g, c->Kx[sr], t.p + c0, Wr);
+                    g.alpha = 0.5;
+                    run(c, g);
+                    {   // + Xd[(m,e),(j,b)] = sum_Q L~_mj L~_be, j in the slab
+                        TcGemm h = G0(o * (j1 - j0), v * v, NQ);
+                        setA(h, n, 1, j1 - j0, 0, nn, 0, 0);
+                        setB(h, 0, nn, n, 1, v, 1);
+                        setC(h, (long long)v * ldW, v, 1, ldW);
+                        ops_cc(h, c->Lt[sr] + j0, plane, c->Lt[sr] + (long long)o * n + o, plane, Wr, wc);
+                        h.beta = 1.0;
+                        run(c, h);
+                    }
+                    EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[sr], o, c->Ft[sr], o, c->Wslab, ldW, wc,
+                       rowoff[sr], -c0, j0, j1);
+                } else {
+                    TcGemm g = G0((int)n1s_[sr], (int)wc, (int)n1s_[sr]);
+                    setA(g, 0, n1s_[sr], 0, (long long)t.Rlo, 1, t.Rlo, 1);
+                    setB(g, t.r_hi, t.r_lo, t.c_hi, t.c_lo, t.Clo, t.c_lo < t.r_lo);
+                    setC(g, 0, ldW, t.Clo, 1);
+                    ops_rc(g, c->Kx[sr], t.p + (long long)j0 * t.c_hi, t.pim, Wr, wc);
+                    g.alpha = 0.5;
+                    run(c, g);
+                }
+            }
+            {   // Z slab = 1/2 N^T N[:, slab]
+                TcGemm g = G0(n1, (int)wc, NQ);
+                setA(g, 0, 1, 0, 0, ld1, 0, 0);
+                setB(g, 0, ld1, 0, 1, 0, 1);
+                setC(g, 0, ldW, 0, 1);
+                ops_cc(g, c->Nq, n1, c->Nq + rowoff[sc] + c0, n1, c->Zslab, wc);
+                g.alpha = 0.5;
+                run(c, g);
+            }
+            for (int sr = 0; sr < 2; ++sr) {
+                if (n1s_[sr] == 0) continue;
+                for (int sk = 0; sk < 2; ++sk) {
+                    if (n1s_[sk] == 0) continue;
+                    const TOp t = t_block(c, x, sr, sk);
+                    TcGemm g = G0((int)n1s_[sr], (int)wc, (int)n1s_[sk]);
+                    if (sr == sk) { setA(g, 0, t.r_lo, 0, 0, 1, 0, 1); setB(g, 0, ldW, 0, 1, 0, 1); }
+                    else { setA(g, t.r_hi, t.r_lo, t.Rlo, t.c_hi, t.c_lo, t.Clo, t.c_lo < t.r_lo); setB(g, (long long)t.Clo * ldW, ldW, 0, 1, 0, 1); }
+                    setC(g, sr == sk ? 0 : (long long)t.Rlo * ldW, ldW, 0, 1);
+                    ops_cc(g, t.p, t.pim, c->Wslab + rowoff[sk] * ldW, wc, c->Zslab + rowoff[sr] * ldW, wc);
+                    g.alpha = -1.0; g.beta = 1.0;
+                    run(c, g);
+                }
+            }
+            EW(c, k_fold_slab, d.n_t2, d, sc, j0, j1, c->Zslab, wc, c->opairs[sc], c->vpairs[sc], r + 2 * d.n_t1);
+        }
+    }
+
+    // ---- 10. spin-flip sector with T_AB[(i,B),(M,e)] = -t_iM^eB read from the packed block (sign folded into alpha)
+    c->sec = 10;
+    if (d.nA > 0 && d.nB > 0) {
+        const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], nA = d.nA, nB = d.nB;
+        const long long lA = 2LL * nA, lB = 2LL * nB;
+        const double* tp = x + 2 * d.n_t1 + 2 * d.off_t2[2];
+        const long long rI = 2LL * ob * va * vb, rB = 2, cM = 2LL * va * vb, cE = 2LL * vb;      // strides of i, B, M, e
+        double *W = c->Wsf, *Z = c->Zsf;
+        {   // W_BB = 1/2 Kx_BA T_AB
+            TcGemm g = G0(nB, nB, nA);
+            setA(g, 0, nA, 0, vb, 1, vb, 1);
+            setB(g, rI, rB, cM, cE, va, 0);
+            setC(g, 0, lB, va, 1);
+            ops_rc(g, c->KxBA, tp, 1, W, nB);
+            g.alpha = -0.5;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(ob * ob, va * va, NQ);
+            setA(g, n, 1, ob, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, va, 1);
+            setC(g, va * lB, va, 1, lB);
+            ops_cc(g, c->Lt[1], plane, c->Lt[0] + (long long)oa * n + oa, plane, W, nB);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, W, lB, (long long)nB, 0LL, 0LL, 0, ob);
+        {   // Z_AB = -T_AB W_BB
+            TcGemm g = G0(nA, nB, nB);
+            setA(g, rI, rB, vb, cM, cE, va, 0);
+            setB(g, (long long)va * lB, lB, 0, 1, 0, 1);
+            setC(g, (long long)vb * lB, lB, 0, 1);
+            ops_cc(g, tp, 1, W, nB, Z, nB);
+            g.alpha = 1.0;
+            run(c, g);
+        }
+        EW(c, k_fold_slab, d.n_t2, d, 2, 0, 0, Z, (long long)nB, c->opairs[0], c->vpairs[0], r + 2 * d.n_t1);
+        {   // W_AA = 1/2 Kx_BA^T T_AB^T
+            TcGemm g = G0(nA, nA, nB);
+            setA(g, 0, 1, 0, (long long)va * nA, nA, va, 0);
+            setB(g, cM, cE, rI, rB, vb, 1);
+            setC(g, 0, lA, vb, 1);
+            ops_rc(g, c->KxBA, tp, 1, W, nA);
+            g.alpha = -0.5;
+            run(c, g);
+        }
+        {
+            TcGemm g = G0(oa * oa, vb * vb, NQ);
+            setA(g, n, 1, oa, 0, nn, 0, 0);
+            setB(g, 0, nn, n, 1, vb, 1);
+            setC(g, vb * lA, vb, 1, lA);
+            ops_cc(g, c->Lt[0], plane, c->Lt[1] + (long long)ob * n + ob, plane, W, nA);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        EW(c, k_add_Fd, (long long)oa * vb * vb + (long long)oa * oa * vb, oa, vb, n, c->Ft[0], oa, c->Ft[1], ob, W, lA, (long long)nA, 0LL, 0LL, 0, oa);
+        {   // Z_BA = -T_AB^T W_AA
+            TcGemm g = G0(nB, nA, nA);
+            setA(g, cM, cE, va, rI, rB, vb, 1);
+            setB(g, (long long)vb * lA, lA, 0, 1, 0, 1);
+            setC(g, (long long)va * lA, lA, 0, 1);
+            ops_cc(g, tp, 1, W, nA, Z, nA);
+            g.alpha = 1.0;
+            run(c, g);
+        }
+        EW(c, k_fold_slab, d.n_t2, d, 3, 0, 0, Z, (long long)nA, c->opairs[0], c->vpairs[0], r + 2 * d.n_t1);
+    }
+
+    // ---- 11. ladder phase: the arena now holds the tile-major amplitudes and the ladder outputs
+    c->sec = 11;
+    if (d.oo > 0) {
+        CK(cudaMemsetAsync(c->Xt_ab, 0, (size_t)c->xt_ab_cnt * 8, STL));
+        EW(c, k_build_Xt_ab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab);
+    }
+    for (int s = 0; s < 2; ++s)
+        if (d.po[s] > 0) {
+            CK(cudaMemsetAsync(c->Xt_ss[s], 0, (size_t)c->xt_ss_cnt[s] * 8, STL));
+            EW(c, k_build_Xt_ss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->opairs[s], c->Xt_ss[s], (d.v[s] + 7) / 8,
+               (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s]);
+        }
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], STL));
+    c->launches += ladder_launch(c->lb, STL, c->num_sms);
+    c->flops += ladder_flops(c->lb);
+    c->lad_flops = ladder_flops(c->lb);
+    if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], STL));
+
+    if (d.oo > 0) {
+        const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1], oo = d.oo;
+        const long long lY = 2LL * oo;
+        const double* tp = x + 2 * d.n_t1 + 2 * d.off_t2[2];
+        double* Yvv = c->Yab + ((long long)oa * n + ob) * lY;
+        EW(c, k_add_oo_rows, (long long)oo * lY, oa, ob, n, (long long)oo, c->Wooab, c->Yab, c->Voo);
+        {   // + t_mN^aB ( <mN||iJ>~ + Y_iJ^mN )      (the t1 t1 part of tau goes through the rows (m,B) below)
+            TcGemm g = G0(va * vb, oo, oo);
+            setA(g, 2LL * vb, 2, vb, 0, 2LL * va * vb, 0, 0);
+            setB(g, 0, lY, 0, 1, 0, 1);
+            setC(g, n * lY, lY, 0, 1);
+            ops_cc(g, tp, 1, c->Voo, oo, Yvv, oo);
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // rows (m,B): Y^{mB} -= sum_N t_N^B Y^{mN}   (batched over m)
+            TcGemm g = G0(vb, oo, ob);
+            setA(g, 0, 1, 0, 0, vb, 0, 0);
+            setB(g, 0, lY, 0, 1, 0, 1);
+            setC(g, 0, lY, 0, 1);
+            ops_cc(g, c->t1r + d.n1a, n1, c->Yab, oo, c->Yab + (long long)ob * lY, oo);
+            g.nsb = oa; g.sbA = 0; g.sbB = n * lY; g.sbC = n * lY;
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {   // - sum_m t_m^a Y_iJ^mB
+            TcGemm g = G0(va, vb * oo, oa);
+            setA(g, 0, 1, 0, 0, va, 0, 0);
+            setB(g, 0, n * lY, lY, 1, oo, 1);
+            setC(g, 0, n * lY, lY, 1);
+            ops_cc(g, c->t1r, n1, c->Yab + (long long)ob * lY, oo, Yvv, oo);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {   // - sum_N t_N^B Y_iJ^aN   (batched over a)
+            TcGemm g = G0(vb, oo, ob);
+            setA(g, 0, 1, 0, 0, vb, 0, 0);
+            setB(g, 0, lY, 0, 1, 0, 1);
+            setC(g, 0, lY, 0, 1);
+            ops_cc(g, c->t1r + d.n1a, n1, c->Yab + (long long)oa * n * lY, oo, Yvv, oo);
+            g.nsb = va; g.sbA = 0; g.sbB = n * lY; g.sbC = n * lY;
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+    }
+    for (int s = 0; s < 2; ++s) {
+        const int o = d.o[s], v = d.v[s], po = d.po[s], pv = d.pv[s];
+        const long long off1 = rowoff[s];
+        if (po == 0 || pv == 0) continue;
+        const long long lP = 2LL * po;
+        const double* tss = t2p + 2 * d.off_t2[s];
+        EW(c, k_ss_prep_lean, (long long)po * po, o, po, n, c->opairs[s], c->W4[s], c->Yss[s], c->Vp[s], c->Yoo[s]);
+        {   // rows (a<b): + t_mn^ab ( <mn||ij>~ + Y_ij^mn ), m<n, straight from the packed block
+            TcGemm g = G0(pv, po, po);
+            setA(g, 0, 2, 0, 0, 2LL * pv, 0, 0);
+            setB(g, 0, lP, 0, 1, 0, 1);
+            setC(g, 0, 0, 0, 1);
+            ops_cc(g, tss, 1, c->Vp[s], po, c->Yss[s], po);
+            g.cm_table = c->cmp[s];
+            g.beta = 1.0;
+            run(c, g);
+        }
+        {   // rows (m,b): Y^{mb} -= 1/2 sum_n t_n^b Y^{mn}   (batched over m; supplies the t1 t1 part of tau)
+            TcGemm g = G0(v, po, o);
+            setA(g, 0, 1, 0, 0, v, 0, 0);
+            setB(g, 0, lP, 0, 1, 0, 1);
+            setC(g, 0, lP, 0, 1);
+            ops_cc(g, c->t1r + off1, n1, c->Yoo[s], po, c->Yss[s] + (long long)o * lP, po);
+            g.nsb = o; g.sbA = 0; g.sbB = (long long)o * lP; g.sbC = n * lP;
+            g.alpha = -0.5; g.beta = 1.0;
+            run(c, g);
+        }
+        double* Yvv = c->Yss[s] + ((long long)o * n + o) * lP;
+        {   // Y^{ab} -= sum_m t_m^a Y^{mb}
+            TcGemm g = G0(v, v * po, o);
+            setA(g, 0, 1, 0, 0, v, 0, 0);
+            setB(g, 0, n * lP, lP, 1, po, 1);
+            setC(g, 0, n * lP, lP, 1);
+            ops_cc(g, c->t1r + off1, n1, c->Yss[s] + (long long)o * lP, po, Yvv, po);
+            g.alpha = -1.0; g.beta = 1.0;
+            run(c, g);
+        }
+        {   // Y^{ab} += sum_m t_m^b Y^{ma}
+            TcGemm g = G0(v, v * po, o);
+            setA(g, 0, 1, 0, 0, v, 0, 0);
+            setB(g, 0, n * lP, lP, 1, po, 1);
+            setC(g, 0, lP, n * lP, 1);
+            ops_cc(g, c->t1r + off1, n1, c->Yss[s] + (long long)o * lP, po, Yvv, po);
+            g.beta = 1.0;
+            run(c, g);
+        }
+    }
+
+    // ---- 12. ladder pieces and singles into the packed residual
+    c->sec = 12;
+    {
+        AsmArgs A;
+        memset(&A, 0, sizeof(A));
+        A.Yab = c->Yab; A.r1buf = c->r1buf;
+        for (int s = 0; s < 2; ++s) { A.Yss[s] = c->Yss[s]; A.Ft[s] = c->Ft[s]; A.opairs[s] = c->opairs[s]; A.vpairs[s] = c->vpairs[s]; }
+        A.r1p = r; A.r2p = r + 2 * d.n_t1;
+        EW(c, k_fold_ladder, d.n_t1 + d.n_t2, d, A);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { c->cuda_err = (int)e; return RTCC_ECUDA; }
+    return RTCC_OK;
+#undef STL
+}
+
+int run_pipeline(rtcc_ctx* c, const double* x, double* r)
+{ return c->lean ? residual_pipeline_lean(c, x, r) : residual_pipeline(c, x, r); }
+
+}  // namespace
+
+namespace {
+
 int copy_in(rtcc_ctx* c, double* dst, const double* src, long long ndoubles)
 {
     if (ndoubles <= 0) return 0;
@@ -673,7 +1226,7 @@ int eval_gx(rtcc_ctx* c)
         c->flops += c->res_flops;
         return 0;
     }
-    int rc = residual_pipeline(c, c->gx, c->gr);
+    int rc = run_pipeline(c, c->gx, c->gr);
     return rc;
 }
 
@@ -692,6 +1245,89 @@ void model_ladder_flops(rtcc_ctx* c)
     double pva = d.pv[0], pvb = d.pv[1], vab = (double)d.v[0] * d.v[1];
     c->lad_model = 4.0 * (pva * pva * d.po[0] + pvb * pvb * d.po[1] + vab * vab * d.oo)
                  + 2.0 * d.NQ * (2.0 * pva * pva + 2.0 * pvb * pvb + vab * vab);
+}
+
+}  // namespace
+
+
+namespace {
+
+struct SizePlan {
+    long long persistent = 0, arena = 0;       // doubles
+    long long a_lt[2]{}, a_tss[2]{}, a_wslab = 0, a_zslab = 0, a_wsf = 0, a_zsf = 0;      // arena offsets, ring phase
+    long long a_xt_ab = 0, a_xt_ss[2]{}, a_yab = 0, a_yss[2]{};                           // arena offsets, ladder phase
+    long long xt_ab = 0, xt_ss[2]{};
+    int slab_j[2]{1, 1};
+};
+
+// Device memory of a context in doubles, in closed form (tested against rtcc_sizes).  standard: everything resident;
+// lean: persistent part + one arena shared by the ring phase (dressed vectors, same-spin pair-space blocks, one column
+// slab of W and Z, or the spin-flip W and Z) and the ladder phase (tile-major amplitudes and the ladder outputs).
+long long size_plan(const Dims& d, bool lean, int want_slab_j, SizePlan* out)
+{
+    const long long n = d.n, nn = n * n, NQ = d.NQ, plane = NQ * nn, n1 = d.n1, nA = d.nA, nB = d.nB, oo = d.oo;
+    const long long namp = d.n_t1 + d.n_t2;
+    const long long nQt = (NQ + 15) / 16, nPt = (n + 7) / 8;
+    auto al = [](long long x) { return (x + 31) / 32 * 32; };             // cudaMalloc granularity is far coarser; 256 B here
+    SizePlan sp;
+    long long P = 0;
+    long long xt_ss[2], yss[2], tss[2];
+    for (int s = 0; s < 2; ++s) {
+        const long long o = d.o[s], v = d.v[s], po = d.po[s];
+        const long long nt2 = 2 * po <= 64 ? 64 : 128, ncol = (2 * po + nt2 - 1) / nt2;
+        xt_ss[s] = ((v + 15) / 16) * ((v + 7) / 8) * ncol * 128 * (nt2 + 4);
+        yss[s] = nn * 2 * po;
+        tss[s] = 2 * (o * v) * (o * v);
+        P += plane + nn + nn + 2 * nn + (o * v) * (o * v);                  // L, fockd, Fb, Ft, Kx
+        P += nPt * ((v + 15) / 16) * nQt * 16 * LD_LDA1 + nPt * ((v + 7) / 8) * nQt * 16 * LD_LDB1;      // LtA, LtB
+        P += o * o * 2 * o * o + 2 * (po * 2 * po);                        // W4, Wp/Vp, Yoop
+        if (lean) P += o * o * 2 * po + d.pv[s];                           // Yoo, row table
+        else P += 2 * plane + 3 * (v * v * 2 * po) + xt_ss[s] + yss[s];    // Lt, Xss, tauss, Zv, Xt_ss, Yss
+    }
+    const long long nt2ab = 2 * oo <= 64 ? 64 : 128, ncolab = (2 * oo + nt2ab - 1) / nt2ab;
+    const long long xt_ab = ((d.v[0] + 15) / 16) * ((d.v[1] + 7) / 8) * ncolab * 128 * (nt2ab + 4), yab = nn * 2 * oo;
+    P += nB * nA + 2 * n1 + 2 * (2 * NQ * n1) + 2 * NQ + 2 * n1 + oo * 2 * oo;          // KxBA, t1r, Mq, Nq, gam, r1buf, Wooab
+    P += (32LL << 20) + 4 * 2 * namp;                                                    // GEMM workspace, gx, gr, t_cur, r_cur
+    if (lean) P += oo * 2 * oo;                                                           // Voo
+    else P += 3 * (2 * n1 * n1) + 3 * (2 * nA * nB) + 2 * nB * nB + 2 * nA * nA + 2 * ((long long)d.v[0] * d.v[1] * 2 * oo) + xt_ab + yab;
+    sp.persistent = P;
+    sp.xt_ab = xt_ab; sp.xt_ss[0] = xt_ss[0]; sp.xt_ss[1] = xt_ss[1];
+    if (lean) {
+        long long a = 0;
+        for (int s = 0; s < 2; ++s) { sp.a_lt[s] = a; a += al(2 * plane); }
+        const long long after_lt = a;
+        for (int s = 0; s < 2; ++s) { sp.a_tss[s] = a; a += al(tss[s]); }
+        const long long ring_fixed = a;
+        long long c = 0;
+        sp.a_xt_ab = c; c += al(xt_ab);
+        for (int s = 0; s < 2; ++s) { sp.a_xt_ss[s] = c; c += al(xt_ss[s]); }
+        sp.a_yab = c; c += al(yab);
+        for (int s = 0; s < 2; ++s) { sp.a_yss[s] = c; c += al(yss[s]); }
+        const long long ladder_total = c;
+        const long long sf = al(2 * (nB > nA ? nB * nB : nA * nA)) + al(2 * nA * nB);
+        // column slabs: as many occupied indices j per slab as fit beside the fixed part without growing the arena beyond the
+        // ladder phase (at least one)
+        for (int s = 0; s < 2; ++s) {
+            const long long per_j = 2 * (n1 * 2 * d.v[s]);                   // W and Z columns of one j
+            long long room = ladder_total - ring_fixed;
+            long long nj = per_j > 0 ? room / (per_j + 64) : d.o[s];
+            if (nj < 1) nj = 1;
+            if (nj > d.o[s]) nj = d.o[s];
+            if (want_slab_j > 0 && want_slab_j < nj) nj = want_slab_j;
+            if (nj < 1) nj = 1;
+            sp.slab_j[s] = (int)nj;
+        }
+        long long wc = 0;
+        for (int s = 0; s < 2; ++s) { const long long w = (long long)sp.slab_j[s] * d.v[s]; if (w > wc) wc = w; }
+        sp.a_wslab = ring_fixed; sp.a_zslab = ring_fixed + al(n1 * 2 * wc);
+        const long long ring_total = sp.a_zslab + al(n1 * 2 * wc);
+        sp.a_wsf = after_lt; sp.a_zsf = after_lt + al(2 * (nB > nA ? nB * nB : nA * nA));
+        const long long sf_total = after_lt + sf;
+        sp.arena = ring_total > ladder_total ? ring_total : ladder_total;
+        if (sf_total > sp.arena) sp.arena = sf_total;
+    }
+    if (out) *out = sp;
+    return sp.persistent + sp.arena;
 }
 
 }  // namespace
@@ -727,6 +1363,8 @@ int rtcc_set_default_option(const char* name, int value)
     else if (k == "max_cluster") { if (value < 1 || value > 16) return RTCC_EINVAL; g_opt.lad.max_cluster = value; }
     else if (k == "ladder_cluster") { if (value < 0 || value > 16) return RTCC_EINVAL; g_opt.lad.force_cluster = value; }
     else if (k == "ladder_tiles") { if (value < 1 || value > LW_MAXC) return RTCC_EINVAL; g_opt.lad.max_tiles = value; }
+    else if (k == "lean") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.lean = value; }
+    else if (k == "lean_slab") { if (value < 0) return RTCC_EINVAL; g_opt.lean_slab_j = value; }
     else if (k == "reset") g_opt = RtccOptions();
     else return RTCC_EINVAL;
     return RTCC_OK;
@@ -819,22 +1457,53 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
 #endif
         CKC(cudaMallocHost((void**)&c->h_scal, 8 * sizeof(double)));
 
+        // lean or standard layout?
+        {
+            SizePlan sp;
+            const long long std_doubles = size_plan(d, false, 0, nullptr);
+            bool lean = c->opt.lean == 1;
+            if (c->opt.lean == -1) {
+                size_t fr = 0, tot = 0;
+                CKC(cudaMemGetInfo(&fr, &tot));
+                lean = (double)std_doubles * 8.0 > 0.94 * (double)fr;
+            }
+            c->lean = lean;
+            if (lean) {
+                size_plan(d, true, c->opt.lean_slab_j, &sp);
+                c->arena_cap = sp.arena;
+                DA(c->arena, sp.arena, nullptr);
+                c->slab_j[0] = sp.slab_j[0]; c->slab_j[1] = sp.slab_j[1];
+                for (int s = 0; s < 2; ++s) {
+                    c->Lt[s] = c->arena + sp.a_lt[s]; c->Tss[s] = c->arena + sp.a_tss[s];
+                    c->Xt_ss[s] = c->arena + sp.a_xt_ss[s]; c->Yss[s] = c->arena + sp.a_yss[s];
+                    c->xt_ss_cnt[s] = sp.xt_ss[s];
+                }
+                c->Wslab = c->arena + sp.a_wslab; c->Zslab = c->arena + sp.a_zslab;
+                c->Wsf = c->arena + sp.a_wsf; c->Zsf = c->arena + sp.a_zsf;
+                c->Xt_ab = c->arena + sp.a_xt_ab; c->Yab = c->arena + sp.a_yab;
+                c->xt_ab_cnt = sp.xt_ab;
+                c->fused_fock = false;                       // the fused singles kernel reads the whole pair-space matrix
+                c->named.push_back({"Yab", {c->Yab, (long long)nn * 2 * d.oo}});
+            }
+        }
         for (int s = 0; s < 2; ++s) {
             DA(c->L[s], plane, s ? "L1" : "L0");
-            DA(c->Lt[s], 2 * plane, s ? "Lt1" : "Lt0");
+            if (!c->lean) DA(c->Lt[s], 2 * plane, s ? "Lt1" : "Lt0");
             DA(c->fockd[s], nn, nullptr);
             DA(c->Fb[s], nn, s ? "Fb1" : "Fb0");
             DA(c->Ft[s], 2 * nn, s ? "Ft1" : "Ft0");
             DA(c->Kx[s], (long long)d.o[s] * d.v[s] * d.o[s] * d.v[s], s ? "Kx1" : "Kx0");
             const int po = d.po[s], v = d.v[s], o = d.o[s];
-            DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
+            if (!c->lean) DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
             {
                 const int nt2 = 2 * po <= 64 ? 64 : 128;
                 c->nt2_ss[s] = nt2;
                 const long long ncol = (2 * po + nt2 - 1) / nt2;
                 const long long cx = (long long)((v + 15) / 16) * ((v + 7) / 8) * ncol * 128 * (nt2 + 4);
-                DA(c->Xt_ss[s], cx, nullptr);
-                CKC(cudaMemsetAsync(c->Xt_ss[s], 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+                if (!c->lean) {
+                    DA(c->Xt_ss[s], cx, nullptr);
+                    CKC(cudaMemsetAsync(c->Xt_ss[s], 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+                }
                 const long long nQt = (NQ + 15) / 16, nPt = (n + 7) / 8;
                 const long long ca = nPt * ((v + 15) / 16) * nQt * 16 * LD_LDA1, cb = nPt * ((v + 7) / 8) * nQt * 16 * LD_LDB1;
                 DA(c->LtA[s], ca, nullptr);
@@ -842,24 +1511,32 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 CKC(cudaMemsetAsync(c->LtA[s], 0, (size_t)ca * 8, c->st));
                 CKC(cudaMemsetAsync(c->LtB[s], 0, (size_t)cb * 8, c->st));
             }
-            DA(c->tauss[s], (long long)v * v * 2 * po, nullptr);
-            DA(c->Yss[s], nn * 2 * po, s ? "Yss1" : "Yss0");
             DA(c->W4[s], (long long)o * o * 2 * o * o, nullptr);
             DA(c->Wp[s], (long long)po * 2 * po, nullptr);
             DA(c->Yoop[s], (long long)po * 2 * po, nullptr);
-            DA(c->Zv[s], (long long)v * v * 2 * po, s ? "Zv1" : "Zv0");
-            CKC(cudaMemsetAsync(c->Yss[s], 0, (size_t)(nn * 2 * po > 0 ? nn * 2 * po : 1) * 8, c->st));
+            if (c->lean) {
+                c->Vp[s] = c->Wp[s];
+                DA(c->Yoo[s], (long long)o * o * 2 * po, nullptr);
+                DA(c->cmp[s], d.pv[s], nullptr);
+            } else {
+                DA(c->tauss[s], (long long)v * v * 2 * po, nullptr);
+                DA(c->Yss[s], nn * 2 * po, s ? "Yss1" : "Yss0");
+                DA(c->Zv[s], (long long)v * v * 2 * po, s ? "Zv1" : "Zv0");
+                CKC(cudaMemsetAsync(c->Yss[s], 0, (size_t)(nn * 2 * po > 0 ? nn * 2 * po : 1) * 8, c->st));
+            }
         }
         DA(c->KxBA, (long long)d.nB * d.nA, "KxBA");
         DA(c->t1r, 2LL * n1, "t1r");
-        DA(c->Tsc, 2LL * n1 * n1, "Tsc");
-        DA(c->Wsc, 2LL * n1 * n1, "Wsc");
-        DA(c->Zsc, 2LL * n1 * n1, "Zsc");
-        DA(c->TAB, 2LL * d.nA * d.nB, "TAB");
-        DA(c->WBB, 2LL * d.nB * d.nB, "WBB");
-        DA(c->WAA, 2LL * d.nA * d.nA, "WAA");
-        DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
-        DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
+        if (!c->lean) {
+            DA(c->Tsc, 2LL * n1 * n1, "Tsc");
+            DA(c->Wsc, 2LL * n1 * n1, "Wsc");
+            DA(c->Zsc, 2LL * n1 * n1, "Zsc");
+            DA(c->TAB, 2LL * d.nA * d.nB, "TAB");
+            DA(c->WBB, 2LL * d.nB * d.nB, "WBB");
+            DA(c->WAA, 2LL * d.nA * d.nA, "WAA");
+            DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
+            DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
+        }
         DA(c->Mq, 2LL * NQ * n1, "Mq");
         if (c->fused_fock) {
             DA(c->fockPart, (long long)c->fuse_nch * 8 * nn, nullptr);
@@ -870,17 +1547,21 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->Nq, 2LL * NQ * n1, "Nq");
         DA(c->gam, 2LL * NQ, "gam");
         DA(c->r1buf, 2LL * n1, "r1buf");
-        DA(c->Xab, (long long)va * vb * 2 * d.oo, "Xab");
         {
             const int nt2 = 2 * d.oo <= 64 ? 64 : 128;
             c->nt2_ab = nt2;
             const long long ncol = (2 * d.oo + nt2 - 1) / nt2;
             const long long cx = (long long)((va + 15) / 16) * ((vb + 7) / 8) * ncol * 128 * (nt2 + 4);
-            DA(c->Xt_ab, cx, nullptr);
-            CKC(cudaMemsetAsync(c->Xt_ab, 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+            if (!c->lean) {
+                DA(c->Xt_ab, cx, nullptr);
+                CKC(cudaMemsetAsync(c->Xt_ab, 0, (size_t)(cx > 0 ? cx : 1) * 8, c->st));
+            }
         }
-        DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
-        DA(c->Yab, nn * 2 * d.oo, "Yab");
+        if (!c->lean) {
+            DA(c->Xab, (long long)va * vb * 2 * d.oo, "Xab");
+            DA(c->tauab, (long long)va * vb * 2 * d.oo, nullptr);
+            DA(c->Yab, nn * 2 * d.oo, "Yab");
+        } else DA(c->Voo, (long long)d.oo * 2 * d.oo, nullptr);
         DA(c->Wooab, (long long)d.oo * 2 * d.oo, nullptr);
         c->ws_cap = 32LL << 20;
         DA(c->ws, c->ws_cap, nullptr);
@@ -909,6 +1590,8 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             DA(c->vpairs[s], vp.size(), nullptr);
             CKC(cudaMemcpy(c->opairs[s], op.data(), op.size() * sizeof(int2), cudaMemcpyHostToDevice));
             CKC(cudaMemcpy(c->vpairs[s], vp.data(), vp.size() * sizeof(int2), cudaMemcpyHostToDevice));
+            if (c->lean && d.pv[s] > 0)
+                k_pair_row_table<<<nblk(d.pv[s], 1024), 256, 0, c->st>>>(d.o[s], n, d.pv[s], 2LL * d.po[s], c->vpairs[s], c->cmp[s]);
         }
         {
             std::vector<int2> tab, tss;
@@ -1010,7 +1693,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         // R(T=0), E(T=0); count the launches / flops of one evaluation; then capture it as a graph
         {
             long long l0 = c->launches; double f0 = c->flops;
-            rc = residual_pipeline(c, c->gx, c->gr);
+            rc = run_pipeline(c, c->gx, c->gr);
             if (rc) goto fail;
             c->res_launches = c->launches - l0; c->res_flops = c->flops - f0;
             CKC(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
@@ -1027,7 +1710,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
             int prc = RTCC_OK;
             if (e == cudaSuccess) {
-                prc = residual_pipeline(c, c->gx, c->gr);
+                prc = run_pipeline(c, c->gx, c->gr);
                 e = cudaStreamEndCapture(cs, &gph);
             }
             c->st = user; c->capturing = false;

@@ -38,6 +38,7 @@ struct TcGemm {
     int a_klin, b_klin;                      // k index of A / B is effectively single-level (set by the launcher)
     int ksplit;                              // deterministic split-K (partials in ws, reduced by a 2nd kernel)
     double* ws;
+    const long long* cm_table;               // optional: offset of output row m (replaces the two-level row index of C)
 };
 
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, bool valid)
@@ -292,7 +293,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
     for (int i = 0; i < TM; ++i) {
         int m = m0 + wm0 + 8 * i + lr;
         if (m >= g.M) continue;
-        long long mo = idx2(m, g.Mlo, g.cm_hi, g.cm_lo);
+        long long mo = g.cm_table ? g.cm_table[m] : idx2(m, g.Mlo, g.cm_hi, g.cm_lo);
 #pragma unroll
         for (int j = 0; j < TN; ++j) {
 #pragma unroll
@@ -322,7 +323,7 @@ __global__ void tcgemm_splitk_reduce(const TcGemm g)
         const double* W = g.ws + (long long)bt * g.ksplit * MN + r;
         double s = 0.0;
         for (int k = 0; k < g.ksplit; ++k) s += W[k * MN];
-        double* p = g.C[db] + sb * g.sbC + idx2(m, g.Mlo, g.cm_hi, g.cm_lo) + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+        double* p = g.C[db] + sb * g.sbC + (g.cm_table ? g.cm_table[m] : idx2(m, g.Mlo, g.cm_hi, g.cm_lo)) + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
         double v = g.alpha * s;
         if (g.beta != 0.0) v += g.beta * *p;
         *p = v;
