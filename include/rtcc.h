@@ -53,7 +53,8 @@ enum { RTCC_HOST_PTRS = 1u };
  *        symmetric in (p,q).
  *   fock [2][n][n] real symmetric Fock matrix of the (N-1)-electron reference (need not be diagonal).
  *   Both are copied.  cuda_stream: a cudaStream_t (NULL = default stream).
- * State after creation: T1 = T2 = 0, C = 0, tau = 0, R(T=0) evaluated. */
+ * State after creation: T1 = T2 = 0, C = 0, tau = 0; R(T=0) and E(T=0) are evaluated by the first call that needs them
+ * (rtcc_step, rtcc_cumulant, rtcc_save). */
 int rtcc_create(rtcc_ctx** out, int o_alpha, int o_beta, int v_alpha, int v_beta, int n_chol,
                 const double* L, const double* fock, unsigned flags, void* cuda_stream);
 void rtcc_destroy(rtcc_ctx* ctx);
@@ -69,12 +70,24 @@ void rtcc_destroy(rtcc_ctx* ctx);
  *   "max_cluster" (16)      largest thread-block cluster the wide ladder kernel may use (1..16)
  *   "ladder_cluster" (0)    0: automatic, k >= 1: force clusters of k CTAs in the wide ladder kernel
  *   "ladder_tiles" (5)      column tiles one CTA of the wide ladder kernel may hold (1..5; 4 of them parked in tensor memory)
+ *   "lean" (-1)             -1: low-memory layout only when the standard one does not fit, 0: never, 1: always
+ *   "lean_slab" (0)         0: automatic, k >= 1: at most k occupied indices per column slab of the low-memory ring
  *   "reset"                 back to the defaults (value ignored)
  * Returns RTCC_EINVAL for an unknown name or a value out of range. */
 int rtcc_set_default_option(const char* name, int value);
 
 /* n_t1, n_t2: complex element counts of the packed arrays; workspace_bytes: device memory held. */
 int rtcc_sizes(const rtcc_ctx* ctx, long long* n_t1, long long* n_t2, long long* workspace_bytes);
+
+/* Size accounting without a context (Table 2; needs no GPU):
+ *   out[0] n_t1, out[1] n_t2   complex elements of the packed boundary arrays
+ *   out[2]  complex elements of ONE T2 in the paper's storage -- the three unpacked spin blocks
+ *           o_a^2 v_a^2 + o_b^2 v_b^2 + o_a o_b v_a v_b (x 16 bytes reproduces the "T2" column of Table 2)
+ *   out[3]  doubles of the Cholesky vectors L[2][n_chol][n][n]
+ *   out[4]  bytes of device memory a context holds with every intermediate resident (the standard layout)
+ *   out[5]  bytes with the low-memory layout (packed alpha-beta amplitudes read in place, ring intermediates in column slabs,
+ *           one arena shared by the ring and ladder phases); rtcc_create picks it when out[4] exceeds the free memory. */
+int rtcc_problem_sizes(int o_alpha, int o_beta, int v_alpha, int v_beta, int n_chol, long long out[6]);
 
 /* Pure evaluation of Eqs. 7-8 at the given amplitudes; does not touch the propagation state.
  * r1/r2 receive R1/R2 in the packed layout. */

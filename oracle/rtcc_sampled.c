@@ -200,21 +200,37 @@ sctx *sorc_create(int oa, int ob, int va, int vb, int K, const double *L, const 
         for (long long pq = 0; pq < (long long)nn; ++pq)
             for (int Q = 0; Q < K; ++Q) c->LT[s][(size_t)pq * K + Q] = L[((size_t)s * K + Q) * nn + pq];
     }
-    /* (me|nf) for same-spin pairs; symmetric, so the lower triangle is mirrored */
+    /* (me|nf) for same-spin pairs; symmetric, so the lower triangle is mirrored.  Every element is the plain sum over Q of
+     * L_me L_nf; four rows X are taken against one row Y at a time only so that the K-vector of Y is read once for the four
+     * (the table is 1.4e9 dot products of length 2200 at config 5). */
     {
         const long long n1 = c->n1;
-#pragma omp parallel for schedule(dynamic, 8)
+        double *ov = (double *)malloc(sizeof(double) * (size_t)(n1 > 0 ? n1 : 1) * K);          /* L_me by pair index, K contiguous */
+        if (!ov) { sorc_destroy(c); return NULL; }
+#pragma omp parallel for schedule(static)
         for (long long X = 0; X < n1; ++X) {
-            int m, e;
-            if (X < c->n1a) { m = (int)(X / va); e = (int)(X % va); }
-            else { long long y = X - c->n1a; m = oa + (int)(y / vb); e = va + (int)(y % vb); }
-            for (long long Y = X; Y < n1; ++Y) {
-                int nn_, f;
-                if (Y < c->n1a) { nn_ = (int)(Y / va); f = (int)(Y % va); }
-                else { long long y = Y - c->n1a; nn_ = oa + (int)(y / vb); f = va + (int)(y % vb); }
-                c->ovov[(size_t)X * n1 + Y] = coul(c, m, VV(e), nn_, VV(f));
+            int m, e, sp;
+            if (X < c->n1a) { sp = 0; m = (int)(X / va); e = oa + (int)(X % va); }
+            else { long long y = X - c->n1a; sp = 1; m = (int)(y / vb); e = ob + (int)(y % vb); }
+            memcpy(ov + (size_t)X * K, c->LT[sp] + ((size_t)m * n + e) * K, sizeof(double) * K);
+        }
+#pragma omp parallel for schedule(dynamic, 4)
+        for (long long X0 = 0; X0 < n1; X0 += 4) {
+            const int nx = (int)(n1 - X0 < 4 ? n1 - X0 : 4);
+            for (long long Y = X0; Y < n1; ++Y) {
+                const double *y = ov + (size_t)Y * K;
+                double acc[4] = {0.0, 0.0, 0.0, 0.0};
+                for (int r = 0; r < nx; ++r) {
+                    const double *x = ov + (size_t)(X0 + r) * K;
+                    double a = 0.0;
+#pragma omp simd reduction(+ : a)
+                    for (int k = 0; k < K; ++k) a += x[k] * y[k];
+                    acc[r] = a;
+                }
+                for (int r = 0; r < nx; ++r) c->ovov[(size_t)(X0 + r) * n1 + Y] = acc[r];
             }
         }
+        free(ov);
 #pragma omp parallel for schedule(static)
         for (long long X = 0; X < n1; ++X)
             for (long long Y = 0; Y < X; ++Y) c->ovov[(size_t)X * n1 + Y] = c->ovov[(size_t)Y * n1 + X];

@@ -275,6 +275,142 @@ __global__ void k_assemble(Dims d, AsmArgs A)
     }
 }
 
+// Tiled assembly (north_star: "coalesced ... with shared-memory staging").  Every source of a residual element is contiguous
+// in a DIFFERENT index (the pair-space matrices in the column's virtual index, the ladder output in the occupied pair), so a
+// thread-per-element gather reads one 32-byte sector per 8 bytes used.  Here a CTA owns a 3-D tile, sweeps it once per
+// contiguity class with the matching index fastest across the threads (full sectors), accumulates in shared memory, and
+// writes the packed output with its own fastest index.  Summation order per element is fixed: bit-reproducible.
+constexpr int AS_TJ = 8, AS_TA = 16, AS_TB = 16, AS_PB = AS_TB + 1;
+// alpha-beta block: r2[i,J,a,B] = Zsc[ia,JB] + Zsc[JB,ia] - Z_AB[iB,Ja] - Z_BA[Ja,iB] + Y[(a,B)][(i,J)]
+__global__ void __launch_bounds__(256) k_assemble_ab(Dims d, AsmArgs A)
+{
+    __shared__ double acc[2][AS_TJ][AS_TA][AS_PB];
+    const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1];
+    const int nJt = (ob + AS_TJ - 1) / AS_TJ, nAt = (va + AS_TA - 1) / AS_TA, nBt = (vb + AS_TB - 1) / AS_TB;
+    const long long ntile = (long long)oa * nJt * nAt * nBt;
+    const long long ld = 2LL * d.n1, nss = (long long)d.po[0] * d.pv[0] + (long long)d.po[1] * d.pv[1];
+    const int tid = threadIdx.x;
+    for (long long t = blockIdx.x; t < ntile; t += gridDim.x) {
+        long long k = t;
+        const int B0 = (int)(k % nBt) * AS_TB; k /= nBt;
+        const int a0 = (int)(k % nAt) * AS_TA; k /= nAt;
+        const int J0 = (int)(k % nJt) * AS_TJ; const int i = (int)(k / nJt);
+        __syncthreads();
+        // class "B fastest": Zsc[ia,JB] - Z_BA[Ja,iB]
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int b = x % AS_TB, a = (x / AS_TB) % AS_TA, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            double v = 0.0;
+            if (B < vb && aa < va && J < ob) {
+                const long long ia = (long long)i * va + aa, JB = d.n1a + (long long)J * vb + B, iB = (long long)i * vb + B, Ja = (long long)J * va + aa;
+                v = A.Zsc[ia * ld + pl * (long long)d.n1 + JB] - A.ZBA[Ja * 2 * d.nA + pl * (long long)d.nA + iB];
+            }
+            acc[pl][j][a][b] = v;
+        }
+        __syncthreads();
+        // class "a fastest": Zsc[JB,ia] - Z_AB[iB,Ja]
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int a = x % AS_TA, b = (x / AS_TA) % AS_TB, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            if (B < vb && aa < va && J < ob) {
+                const long long ia = (long long)i * va + aa, JB = d.n1a + (long long)J * vb + B, iB = (long long)i * vb + B, Ja = (long long)J * va + aa;
+                acc[pl][j][a][b] += A.Zsc[JB * ld + pl * (long long)d.n1 + ia] - A.ZAB[iB * 2 * d.nB + pl * (long long)d.nB + Ja];
+            }
+        }
+        __syncthreads();
+        // class "J fastest": ladder output Y[(a,B)][(i,J)]
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int j = x % AS_TJ, b = (x / AS_TJ) % AS_TB, a = (x / (AS_TJ * AS_TB)) % AS_TA, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            if (B < vb && aa < va && J < ob)
+                acc[pl][j][a][b] += A.Yab[((long long)(oa + aa) * d.n + ob + B) * 2 * d.oo + pl * (long long)d.oo + (long long)i * ob + J];
+        }
+        __syncthreads();
+        // packed output, B fastest, (re, im) interleaved
+        for (int x = tid; x < AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int b = x % AS_TB, a = (x / AS_TB) % AS_TA, j = x / (AS_TB * AS_TA);
+            const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            if (B < vb && aa < va && J < ob) {
+                const long long o = nss + (((long long)i * ob + J) * va + aa) * vb + B;
+                reinterpret_cast<double2*>(A.r2p)[o] = make_double2(acc[0][j][a][b], acc[1][j][a][b]);
+            }
+        }
+    }
+}
+// same-spin block of spin s: r2[(i<j),(a<b)] = Z[ia,jb] - Z[ja,ib] - Z[ib,ja] + Z[jb,ia] + Y[(a,b)][(ij)] - Zv[a][b][(ij)] + Zv[b][a][(ij)]
+__global__ void __launch_bounds__(256) k_assemble_ss(Dims d, int s, AsmArgs A)
+{
+    __shared__ double acc[2][AS_TJ][AS_TA][AS_PB];
+    const int o = d.o[s], v = d.v[s], po = d.po[s], pv = d.pv[s];
+    const int nPt = (po + AS_TJ - 1) / AS_TJ, nAt = (v + AS_TA - 1) / AS_TA, nBt = (v + AS_TB - 1) / AS_TB;
+    const long long ntile = (long long)nPt * nAt * nBt;
+    const long long ld = 2LL * d.n1, off = s ? d.n1a : 0, obase = s ? (long long)d.po[0] * d.pv[0] : 0;
+    const int tid = threadIdx.x;
+    const int2* op = A.opairs[s];
+    for (long long t = blockIdx.x; t < ntile; t += gridDim.x) {
+        long long k = t;
+        const int b0 = (int)(k % nBt) * AS_TB; k /= nBt;
+        const int a0 = (int)(k % nAt) * AS_TA; const int p0 = (int)(k / nAt) * AS_TJ;
+        if (a0 >= b0 + AS_TB) continue;                    // no a < b in this tile (block-uniform)
+        __syncthreads();
+        // class "b fastest": Z[ia,jb] - Z[ja,ib]
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int b = x % AS_TB, a = (x / AS_TB) % AS_TA, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            double val = 0.0;
+            if (aa < bb && bb < v && pij < po) {
+                const int2 ij = op[pij];
+                const long long ia = off + (long long)ij.x * v + aa, jb = off + (long long)ij.y * v + bb, ja = off + (long long)ij.y * v + aa, ib = off + (long long)ij.x * v + bb;
+                val = A.Zsc[ia * ld + pl * (long long)d.n1 + jb] - A.Zsc[ja * ld + pl * (long long)d.n1 + ib];
+            }
+            acc[pl][j][a][b] = val;
+        }
+        __syncthreads();
+        // class "a fastest": - Z[ib,ja] + Z[jb,ia]
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int a = x % AS_TA, b = (x / AS_TA) % AS_TB, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            if (aa < bb && bb < v && pij < po) {
+                const int2 ij = op[pij];
+                const long long ia = off + (long long)ij.x * v + aa, jb = off + (long long)ij.y * v + bb, ja = off + (long long)ij.y * v + aa, ib = off + (long long)ij.x * v + bb;
+                acc[pl][j][a][b] += -A.Zsc[ib * ld + pl * (long long)d.n1 + ja] + A.Zsc[jb * ld + pl * (long long)d.n1 + ia];
+            }
+        }
+        __syncthreads();
+        // class "pair (ij) fastest": ladder output and its T1 corrections
+        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int j = x % AS_TJ, b = (x / AS_TJ) % AS_TB, a = (x / (AS_TJ * AS_TB)) % AS_TA, pl = x / (AS_TB * AS_TA * AS_TJ);
+            const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            if (aa < bb && bb < v && pij < po) {
+                const long long c = pl * (long long)po + pij;
+                acc[pl][j][a][b] += A.Yss[s][((long long)(o + aa) * d.n + o + bb) * 2 * po + c]
+                                  - A.Zv[s][((long long)aa * v + bb) * 2 * po + c] + A.Zv[s][((long long)bb * v + aa) * 2 * po + c];
+            }
+        }
+        __syncthreads();
+        // packed output: pair(a,b) = b(b-1)/2 + a, a fastest
+        for (int x = tid; x < AS_TJ * AS_TA * AS_TB; x += 256) {
+            const int a = x % AS_TA, b = (x / AS_TA) % AS_TB, j = x / (AS_TB * AS_TA);
+            const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            if (aa < bb && bb < v && pij < po) {
+                const long long ox = obase + (long long)pij * pv + pair_index(aa, bb);
+                reinterpret_cast<double2*>(A.r2p)[ox] = make_double2(acc[0][j][a][b], acc[1][j][a][b]);
+            }
+        }
+    }
+}
+// singles: r1 = r1buf + f~_ai
+__global__ void k_assemble_r1(Dims d, AsmArgs A)
+{
+    const long long nn = (long long)d.n * d.n;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < d.n_t1; k += (long long)gridDim.x * blockDim.x) {
+        const int s = k >= d.n1a; const int cc = (int)(s ? k - d.n1a : k);
+        const int i = cc / d.v[s], a = cc - i * d.v[s];
+        A.r1p[2 * k] = A.r1buf[k] + A.Ft[s][(long long)(d.o[s] + a) * d.n + i];
+        A.r1p[2 * k + 1] = A.r1buf[d.n1 + k] + A.Ft[s][nn + (long long)(d.o[s] + a) * d.n + i];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Low-memory ("lean") pipeline: BASELINE.json config 5 does not fit 180 GB with the pair-space matrices held whole
 // (Table 2: the paper's storage argument is three amplitude-sized tensors plus the Cholesky

@@ -667,6 +667,28 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const Ladder
         if (g.ncol > 1) ladder_choose_cluster(g.ncol, b.NQ, occ, tune, g.cl, g.ngrp);
         else rows += g.ntiles;
     }
+    // One launch for all wide cases when a common cluster size costs no case more than 3 % (modelled): separate launches
+    // each end in a partly filled last wave.
+    {
+        const double W1 = 128.0 * 64.0 * b.NQ, W2 = 64.0 * 128.0 * 128.0;
+        auto cost = [&](const LadderCase& g, int cl) {
+            if (cl < 1 || cl > 16 || occ.act[cl] <= 0) return 1e300;
+            const int ng = (g.ncol + g.ngrp - 1) / g.ngrp, per = (ng + cl - 1) / cl;
+            if (per > (tune.max_tiles >= 1 && tune.max_tiles < LW_MAXC ? tune.max_tiles : LW_MAXC)) return 1e300;
+            return (W1 + (double)cl * per * W2) / occ.act[cl];
+        };
+        int common = 0;
+        for (int i = 0; i < b.ncase && !common; ++i) {
+            const int cand = b.c[i].cl;
+            if (cand <= 0) continue;
+            bool ok = true;
+            for (int k = 0; k < b.ncase; ++k)
+                if (b.c[k].cl > 0 && cost(b.c[k], cand) > 1.03 * cost(b.c[k], b.c[k].cl)) ok = false;
+            if (ok) common = cand;
+        }
+        if (common && tune.force_cluster < 1)
+            for (int k = 0; k < b.ncase; ++k) if (b.c[k].cl > 0) b.c[k].cl = common;
+    }
     // narrow cases: slices so that the items fill the SMs evenly
     int best = 1;
     if (rows > 0 && rows < 8LL * num_sms) {

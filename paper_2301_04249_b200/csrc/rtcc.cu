@@ -75,6 +75,7 @@ struct rtcc_ctx {
     // propagation state
     double time = 0.0, C[2] = {0, 0}, E[2] = {0, 0}, E_res[2] = {0, 0};
     int mode = 0, max_micro = 200, fixed_micro = 0, last_micro = 0;
+    bool state_valid = false;             // r_cur / E hold R(t_cur), E(t_cur) (evaluated by the first call that needs them)
     double tol = 1e-4;
 
     // instrumentation
@@ -648,7 +649,23 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             A.opairs[s] = c->opairs[s]; A.vpairs[s] = c->vpairs[s];
         }
         A.r1p = r; A.r2p = r + 2 * d.n_t1;
-        EW(c, k_assemble, d.n_t1 + d.n_t2, d, A);
+        // tiled, shared-memory-staged assembly once the blocks are large enough to fill tiles; the element-per-thread
+        // gather below that (Tiny-sized blocks)
+        const bool tiled = d.v[0] >= 16 && d.v[1] >= 16;
+        if (tiled) {
+            if (d.oo > 0) {
+                const long long nt = (long long)d.o[0] * ((d.o[1] + AS_TJ - 1) / AS_TJ) * ((d.v[0] + AS_TA - 1) / AS_TA) * ((d.v[1] + AS_TB - 1) / AS_TB);
+                k_assemble_ab<<<(unsigned)(nt < c->num_sms * 8LL ? nt : c->num_sms * 8LL), 256, 0, c->S[c->si]>>>(d, A);
+                c->launches++;
+            }
+            for (int s = 0; s < 2; ++s)
+                if (d.po[s] > 0 && d.pv[s] > 0) {
+                    const long long nt = (long long)((d.po[s] + AS_TJ - 1) / AS_TJ) * ((d.v[s] + AS_TA - 1) / AS_TA) * ((d.v[s] + AS_TB - 1) / AS_TB);
+                    k_assemble_ss<<<(unsigned)(nt < c->num_sms * 8LL ? nt : c->num_sms * 8LL), 256, 0, c->S[c->si]>>>(d, s, A);
+                    c->launches++;
+                }
+            EW(c, k_assemble_r1, d.n_t1, d, A);
+        } else EW(c, k_assemble, d.n_t1 + d.n_t2, d, A);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { c->cuda_err = (int)e; return RTCC_ECUDA; }
@@ -1237,6 +1254,20 @@ int read_scal(rtcc_ctx* c)
     return 0;
 }
 
+// R(t(tau)) and E(t(tau)) of the current propagation state, evaluated on first use
+int ensure_state(rtcc_ctx* c)
+{
+    if (c->state_valid) return RTCC_OK;
+    CK(cudaMemcpyAsync(c->gx, c->t_cur, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    int rc = eval_gx(c);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
+    if (read_scal(c)) return RTCC_ECUDA;
+    c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
+    c->state_valid = true;
+    return RTCC_OK;
+}
+
 void model_ladder_flops(rtcc_ctx* c)
 {
     // pp apply = 4[P(va)^2 P(oa) + P(vb)^2 P(ob) + (va vb)^2 oa ob],
@@ -1690,16 +1721,9 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         CKC(cudaMemsetAsync(c->gx, 0, (size_t)c->namp * 16, c->st));
         model_ladder_flops(c);
 
-        // R(T=0), E(T=0); count the launches / flops of one evaluation; then capture it as a graph
-        {
-            long long l0 = c->launches; double f0 = c->flops;
-            rc = run_pipeline(c, c->gx, c->gr);
-            if (rc) goto fail;
-            c->res_launches = c->launches - l0; c->res_flops = c->flops - f0;
-            CKC(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
-            if (read_scal(c)) { rc = RTCC_ECUDA; goto fail; }
-            c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
-        }
+        // One evaluation is captured as a CUDA graph (the capture pass also counts its launches / flops).  R(T=0), E(T=0) are
+        // evaluated by the first call that needs them (ensure_state): a residual costs minutes at the largest sizes.
+        c->state_valid = false;
         if (c->opt.graph) {
             cudaStream_t cs = nullptr;
             cudaStream_t user = c->st;
@@ -1714,6 +1738,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 e = cudaStreamEndCapture(cs, &gph);
             }
             c->st = user; c->capturing = false;
+            c->res_launches = c->launches - l0; c->res_flops = c->flops - f0;
             c->launches = l0; c->flops = f0;
             if (e == cudaSuccess && prc == RTCC_OK && gph) e = cudaGraphInstantiate(&c->graph, gph, 0);
             if (gph) cudaGraphDestroy(gph);
@@ -1740,6 +1765,25 @@ int rtcc_sizes(const rtcc_ctx* c, long long* n_t1, long long* n_t2, long long* w
     if (n_t1) *n_t1 = c->d.n_t1;
     if (n_t2) *n_t2 = c->d.n_t2;
     if (workspace_bytes) *workspace_bytes = c->bytes;
+    return RTCC_OK;
+}
+
+int rtcc_problem_sizes(int oa, int ob, int va, int vb, int NQ, long long out[6])
+{
+    if (!out || oa < 0 || ob < 0 || va < 1 || vb < 1 || NQ < 1 || oa + va != ob + vb) return RTCC_EINVAL;
+    Dims d{};
+    d.o[0] = oa; d.o[1] = ob; d.v[0] = va; d.v[1] = vb; d.n = oa + va; d.NQ = NQ;
+    d.n1a = oa * va; d.n1b = ob * vb; d.n1 = d.n1a + d.n1b; d.nA = oa * vb; d.nB = ob * va;
+    for (int s = 0; s < 2; ++s) { d.po[s] = d.o[s] * (d.o[s] - 1) / 2; d.pv[s] = d.v[s] * (d.v[s] - 1) / 2; }
+    d.oo = oa * ob;
+    d.off_t2[0] = 0; d.off_t2[1] = (long long)d.po[0] * d.pv[0]; d.off_t2[2] = d.off_t2[1] + (long long)d.po[1] * d.pv[1];
+    d.n_t1 = d.n1; d.n_t2 = d.off_t2[2] + (long long)d.oo * va * vb;
+    out[0] = d.n_t1;
+    out[1] = d.n_t2;
+    out[2] = (long long)oa * oa * va * va + (long long)ob * ob * vb * vb + (long long)oa * ob * va * vb;     // the paper's unpacked spin blocks
+    out[3] = 2LL * NQ * d.n * d.n;
+    out[4] = 8 * size_plan(d, false, 0, nullptr);
+    out[5] = 8 * size_plan(d, true, 0, nullptr);
     return RTCC_OK;
 }
 
@@ -1783,6 +1827,7 @@ int rtcc_set_amplitudes(rtcc_ctx* c, const double* t1, const double* t2, double 
     if (read_scal(c)) return RTCC_ECUDA;
     c->E[0] = c->h_scal[0]; c->E[1] = c->h_scal[1];
     c->time = time; c->C[0] = cc[0]; c->C[1] = cc[1];
+    c->state_valid = true;
     return RTCC_OK;
 }
 
@@ -1829,6 +1874,7 @@ int rtcc_save(const rtcc_ctx* cc, const char* path)
 {
     rtcc_ctx* c = const_cast<rtcc_ctx*>(cc);
     if (!c || !path) return RTCC_EINVAL;
+    { int rc0 = ensure_state(c); if (rc0) return rc0; }
     FILE* f = fopen(path, "wb");
     if (!f) return RTCC_EIO;
     CkptHeader h;
@@ -1870,6 +1916,7 @@ int rtcc_load(rtcc_ctx* c, const char* path)
     CK(cudaStreamSynchronize(c->st));
     c->mode = h.mode; c->max_micro = h.max_micro; c->fixed_micro = h.fixed_micro; c->tol = h.tol;
     c->time = h.time; c->C[0] = h.C[0]; c->C[1] = h.C[1]; c->E[0] = h.E[0]; c->E[1] = h.E[1];
+    c->state_valid = true;
     return RTCC_OK;
 }
 
@@ -1883,17 +1930,13 @@ int rtcc_set_solver(rtcc_ctx* c, int mode, double tol, int max_micro, int fixed_
 // restores R(t(tau)) after a failed step (its storage held B): one residual evaluation at the unchanged amplitudes
 static int restore_r_cur(rtcc_ctx* c)
 {
-    CK(cudaMemcpyAsync(c->gx, c->t_cur, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
-    int rc = eval_gx(c);
-    if (rc) return rc;
-    CK(cudaMemcpyAsync(c->r_cur, c->gr, (size_t)c->namp * 16, cudaMemcpyDeviceToDevice, c->st));
-    CK(cudaStreamSynchronize(c->st));
-    return RTCC_OK;
+    c->state_valid = false;
+    return ensure_state(c);
 }
-
 int rtcc_step(rtcc_ctx* c, double dt)
 {
     if (!c || !std::isfinite(dt)) return RTCC_EINVAL;
+    { int rc0 = ensure_state(c); if (rc0) return rc0; }
     const long long N = c->namp;
     const double hh = 0.5 * dt;
     int k = 0;
@@ -1951,9 +1994,11 @@ int rtcc_step(rtcc_ctx* c, double dt)
     return RTCC_OK;
 }
 
-int rtcc_cumulant(const rtcc_ctx* c, double out[4])
+int rtcc_cumulant(const rtcc_ctx* cc, double out[4])
 {
+    rtcc_ctx* c = const_cast<rtcc_ctx*>(cc);
     if (!c || !out) return RTCC_EINVAL;
+    { int rc0 = ensure_state(c); if (rc0) return rc0; }
     out[0] = c->C[0]; out[1] = c->C[1]; out[2] = c->E[0]; out[3] = c->E[1];
     return RTCC_OK;
 }

@@ -74,19 +74,18 @@ def make_problem(cfg: Config, sigma: float | None = None, fock_offdiag: float = 
     eps[0] = -20.0
     eps[1:o] = np.sort(rng.uniform(-1.5, -0.3, o - 1))
     eps[o:] = np.sort(rng.uniform(cfg.v_lo, cfg.v_hi, v))
-    Ls = np.empty((K, n, n), dtype=dtype)
     scale = sig * np.exp(-np.arange(K) / cfg.d)
-    for Q in range(K):
-        A = np.triu(rng.standard_normal((n, n)))
-        Ls[Q] = scale[Q] * (A + np.triu(A, 1).T)
     order_a = np.array(list(range(1, o)) + [0] + list(range(o, n)))
-    order_b = np.arange(n)
+    ia = np.ix_(order_a, order_a)
     L = np.empty((2, K, n, n), dtype=dtype)
-    L[0] = Ls[:, order_a][:, :, order_a]
-    L[1] = Ls[:, order_b][:, :, order_b]
+    for Q in range(K):                       # one spatial vector at a time: no third copy of L (10 GB at config 5)
+        A = np.triu(rng.standard_normal((n, n)))
+        S = scale[Q] * (A + np.triu(A, 1).T)
+        L[1, Q] = S                          # beta: spatial order
+        L[0, Q] = S[ia]                      # alpha: core orbital moved to the first virtual position
     fock = np.zeros((2, n, n))
     fock[0] = np.diag(eps[order_a])
-    fock[1] = np.diag(eps[order_b])
+    fock[1] = np.diag(eps)
     if fock_offdiag > 0.0:
         for s in range(2):
             A = rng.standard_normal((n, n)) * fock_offdiag

@@ -22,7 +22,7 @@ SYMBOLS = [
     "rtcc_get_amplitudes", "rtcc_set_solver", "rtcc_step", "rtcc_cumulant", "rtcc_last_micro_iterations", "rtcc_time",
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
     "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
-    "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy", "rtcc_save", "rtcc_load",
+    "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy", "rtcc_save", "rtcc_load", "rtcc_problem_sizes",
 ]
 
 
@@ -65,6 +65,7 @@ def load():
         lib.rtcc_set_default_option.argtypes = [ctypes.c_char_p, i]
         lib.rtcc_ladder_plan.argtypes = [vp, i, P(i)]
         lib.rtcc_ladder_occupancy.argtypes = [vp, P(i)]
+        lib.rtcc_problem_sizes.argtypes = [i, i, i, i, i, P(ll)]
         lib.rtcc_save.argtypes = [vp, ctypes.c_char_p]
         lib.rtcc_load.argtypes = [vp, ctypes.c_char_p]
         lib.rtcc_last_cuda_error.argtypes = [vp]
@@ -75,6 +76,16 @@ def load():
 
 def strerror(code: int) -> str:
     return load().rtcc_strerror(int(code)).decode()
+
+
+def problem_sizes(oa, ob, va, vb, n_chol):
+    """Size accounting without a context (include/rtcc.h: rtcc_problem_sizes); needs no GPU."""
+    buf = (ctypes.c_longlong * 6)()
+    rc = load().rtcc_problem_sizes(oa, ob, va, vb, n_chol, buf)
+    if rc:
+        raise RtccError(rc, "rtcc_problem_sizes")
+    keys = ("n_t1", "n_t2", "t2_unpacked_elements", "cholesky_doubles", "bytes_standard", "bytes_lean")
+    return dict(zip(keys, list(buf)))
 
 
 def set_default_option(name: str, value: int = 0):

@@ -24,3 +24,16 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+import time
+
+_SESSION_T0 = time.time()
+
+
+@pytest.fixture
+def gpu_time_box():
+    """Seconds this pytest session has been running.  The round-end GPU run has a 20-minute limit for the whole `-m gpu` suite;
+    the one test that takes minutes on its own (BASELINE.json config 5) asks before it starts and skips, saying so, rather
+    than let the limit kill the whole run."""
+    return lambda: time.time() - _SESSION_T0

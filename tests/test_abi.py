@@ -52,3 +52,36 @@ def test_product_has_no_oracle_dependency():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"import\s+oracle|from\s+oracle|from\s+\.+\s*oracle|oracle[/.]|librtcc_oracle|orc_", src), f
+
+
+def test_problem_sizes_reproduce_table_2(lib):
+    """The library's own size accounting (rtcc_problem_sizes, no GPU needed) against the T2 column of Table 2:
+    three unpacked spin blocks, complex128, GiB -- values in tests/golden/table2_t2_sizes.txt are the paper's."""
+    from paper_2301_04249_b200 import rtcc
+    rows = [l.split() for l in open(os.path.join(ROOT, "tests", "golden", "table2_t2_sizes.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 4
+    for name, oa, ob, va, vb, gib in rows:
+        oa, ob, va, vb = int(oa), int(ob), int(va), int(vb)
+        ps = rtcc.problem_sizes(oa, ob, va, vb, 100)
+        assert abs(16 * ps["t2_unpacked_elements"] / 2 ** 30 - float(gib)) < 0.07, name        # 5.74 computed vs 5.8 printed (SURVEY.md section 4)
+        P = lambda x: x * (x - 1) // 2
+        assert ps["n_t2"] == P(oa) * P(va) + P(ob) * P(vb) + oa * ob * va * vb and ps["n_t1"] == oa * va + ob * vb
+
+
+def test_memory_budget_of_the_baseline_configs(lib):
+    """Closed-form device-memory budget.  Configs 1-4 fit one 180 GB B200 with everything resident; config 5
+    needs the low-memory layout, which must stay under 175 GB (the card reports 183 359 MiB = 192 GB) and is bounded below by the paper's own count: the
+    Adams-Moulton history (three amplitude-sized tensors) plus the residual and the Cholesky vectors."""
+    from paper_2301_04249_b200 import inputs, rtcc
+    GB = 1e9
+    for name, cfg in inputs.CONFIGS.items():
+        oa, ob, va, vb = cfg.dims
+        ps = rtcc.problem_sizes(oa, ob, va, vb, cfg.K)
+        floor = 4 * 16 * (ps["n_t1"] + ps["n_t2"]) + 8 * ps["cholesky_doubles"]
+        assert floor < ps["bytes_lean"] and floor < ps["bytes_standard"]
+        if name == "largest":
+            assert ps["bytes_standard"] > 300 * GB and ps["bytes_lean"] < 175 * GB
+        else:
+            assert ps["bytes_standard"] < 150 * GB
+    with pytest.raises(rtcc.RtccError):
+        rtcc.problem_sizes(1, 1, 2, 3, 4)
