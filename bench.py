@@ -242,6 +242,29 @@ def config_block(rtcc, name, stream, flush, peak, with_steps):
     return out
 
 
+def run_profile(args, cfg):
+    """Workload for ncu captures (profiles/*.md name this command): R residual evaluations and ONE Adams-Moulton step of the
+    chosen config, nothing timed; prints a marker line that is not a bench value."""
+    import torch
+    from paper_2301_04249_b200 import build, rtcc
+    torch.cuda.set_device(0)
+    build.build()
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=inputs.stabilised_sigma(cfg))
+    stream = torch.cuda.current_stream()
+    ctx = rtcc.Rtcc(oa, ob, va, vb, K, torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda(), stream=stream.cuda_stream)
+    t1, t2 = inputs.random_amplitudes(cfg)
+    t1d, t2d = torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda()
+    r1d, r2d = torch.empty_like(t1d), torch.empty_like(t2d)
+    for _ in range(args.profile_residuals):
+        ctx.residual(t1d, t2d, r1d, r2d)
+    ctx.set_solver(mode=args.mode, tol=BENCH_TOL, max_micro=200, fixed_micro=max(1, args.fixed_micro))
+    ctx.step(cfg.dt)
+    torch.cuda.synchronize()
+    print(json.dumps({"profile_run": True, "workload": workload_text(cfg, (oa, ob, va, vb)), "residuals": args.profile_residuals,
+                      "steps": 1, "ladder_plan": ctx.ladder_plan(), "not_a_bench_value": True}))
+    ctx.close()
+
+
 def run_ours(args, cfg):
     import torch
     from paper_2301_04249_b200 import build, rtcc
@@ -391,6 +414,8 @@ def main():
     ap.add_argument("--mode", type=int, default=BENCH_MODE, choices=[0, 1],
                     help="0: the paper's plain fixed point of Eq. 9 (default, the headline); 1: denominator-preconditioned (NEXT-1)")
     ap.add_argument("--fixed-micro", type=int, default=None, help="micro-iterations per step (0: iterate to tol 1e-4)")
+    ap.add_argument("--profile-residuals", type=int, default=0,
+                    help="ncu workload: run this many residual evaluations and one step of --config, time nothing, print no bench line")
     args = ap.parse_args()
     if args.fixed_micro is None:
         args.fixed_micro = 0 if args.config in ("tiny", "small") else BENCH_FIXED_MICRO
@@ -404,7 +429,9 @@ def main():
         raise SystemExit(subprocess.call(cmd))
     if world > 1 and args.gpus != world:
         raise SystemExit(f"--gpus {args.gpus} does not match WORLD_SIZE {world}")
-    if args.impl == "reference":
+    if args.profile_residuals > 0:
+        run_profile(args, cfg)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     else:
         run_ours(args, cfg)
