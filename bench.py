@@ -322,33 +322,31 @@ def run_ours(args, cfg):
     plan = ctx.ladder_plan()
     wide = any(p["cluster"] > 0 for p in plan)
 
-    # end to end through the C ABI with HOST buffers: each step the amplitudes come from pinned host memory
-    # (rtcc_set_amplitudes: H2D + R(t)), rtcc_step, and go back (rtcc_get_amplitudes: D2H) with C(t)
+    # end to end through the C ABI with HOST buffers: each step the propagation state (T(tau) and R(T(tau)), PAPER.md:135 -- what
+    # the paper's restart files hold) comes from pinned host memory (rtcc_set_state: H2D), rtcc_step, and the new state goes
+    # back to the host (rtcc_get_state: D2H) with tau, C(t), E(t)
     hctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock, stream=stream.cuda_stream)
     hctx.set_solver(mode=args.mode, tol=BENCH_TOL, max_micro=200, fixed_micro=args.fixed_micro)
     n1, n2 = hctx.n_t1, hctx.n_t2
-    h1 = torch.zeros(n1, dtype=torch.complex128).pin_memory().numpy()
-    h2 = torch.zeros(n2, dtype=torch.complex128).pin_memory().numpy()
-    Ch, tm = 0j, 0.0
+    hs = tuple(torch.zeros(n, dtype=torch.complex128).pin_memory().numpy() for n in (n1, n2, n1, n2))
+    _, _, _, _, tm, Ch, Eh = hctx.get_state(out=hs)
     nst = max(3, min(args.steps, 5 if cfg.name != "small" else 10))
     for it in range(1 + nst):
         if it == 1:
             sync_all()
             t0 = time.perf_counter()
-        hctx.set_amplitudes(h1, h2, tm, Ch)
+        hctx.set_state(hs[0], hs[1], hs[2], hs[3], tm, Ch, Eh)
         hctx.step(cfg.dt)
-        a1, a2 = hctx.get_amplitudes()
-        h1[:] = a1; h2[:] = a2
-        Ch, _ = hctx.cumulant(); tm = hctx.time
+        _, _, _, _, tm, Ch, Eh = hctx.get_state(out=hs)
     torch.cuda.synchronize()
     el = time.perf_counter() - t0
     tt = torch.tensor([el], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    e2e = {"value": world * nst / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": 16 * (n1 + n2),
-           "d2h_bytes_per_step": 16 * (n1 + n2) + 32, "steps": nst,
-           "what": "per step: rtcc_set_amplitudes(host: H2D + R(t)) + rtcc_step + rtcc_get_amplitudes(host: D2H) + rtcc_cumulant, RTCC_HOST_PTRS context; "
-                   "one residual evaluation more per step than the resident loop (R at the uploaded amplitudes)"}
+    e2e = {"value": world * nst / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": 32 * (n1 + n2),
+           "d2h_bytes_per_step": 32 * (n1 + n2) + 40, "steps": nst,
+           "what": "per step: rtcc_set_state(pinned host T and R(T): H2D) + rtcc_step + rtcc_get_state(pinned host: D2H of T, R(T), tau, C, E), "
+                   "RTCC_HOST_PTRS context, wall clock around the loop; same residual evaluations per step as the resident loop"}
     hctx.close()
     workspace = ctx.workspace_bytes
     ctx.close()

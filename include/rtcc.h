@@ -71,6 +71,8 @@ void rtcc_destroy(rtcc_ctx* ctx);
  *   "ladder_cluster" (0)    0: automatic, k >= 1: force clusters of k CTAs in the wide ladder kernel
  *   "ladder_tiles" (5)      column tiles one CTA of the wide ladder kernel may hold (1..5; 4 of them parked in tensor memory)
  *   "lean" (-1)             -1: low-memory layout only when the standard one does not fit, 0: never, 1: always
+ *   "ring_3m" (-1)          complex x complex ring products T.W by three real multiplications instead of four (same result up to
+ *                           rounding): -1 automatic (pair space >= 1536 and the two extra matrices fit), 0 never, 1 always
  *   "lean_slab" (0)         0: automatic, k >= 1: at most k occupied indices per column slab of the low-memory ring
  *   "reset"                 back to the defaults (value ignored)
  * Returns RTCC_EINVAL for an unknown name or a value out of range. */
@@ -108,6 +110,14 @@ int rtcc_get_amplitudes(const rtcc_ctx* ctx, double* t1, double* t2);
  * sizes differ, RTCC_EIO for a short or foreign file; the state is untouched on error).  A loaded run continues bit-identically. */
 int rtcc_save(const rtcc_ctx* ctx, const char* path);
 int rtcc_load(rtcc_ctx* ctx, const char* path);
+
+/* The same state through memory instead of a file (pointer kind as chosen at rtcc_create; scal is a HOST array:
+ * tau, Re C, Im C, Re E, Im E).  rtcc_get_state copies T(tau) -> t1|t2 and R(T(tau)) -> r1|r2 (packed layout);
+ * rtcc_set_state installs them WITHOUT evaluating the residual -- the caller vouches that r1|r2 is R at t1|t2 (as returned
+ * by rtcc_get_state or rtcc_residual); a run continued from a state taken with rtcc_get_state is bit-identical.  Solver
+ * settings are not part of this call (rtcc_set_solver).  RTCC_EINVAL for a NULL pointer or a non-finite scalar. */
+int rtcc_get_state(const rtcc_ctx* ctx, double* t1, double* t2, double* r1, double* r2, double scal[5]);
+int rtcc_set_state(rtcc_ctx* ctx, const double* t1, const double* t2, const double* r1, const double* r2, const double scal[5]);
 
 /* Solver of the implicit Eq. 9.  mode 0: plain fixed point t(k+1) = B + (i dt/2) R(t(k));
  * mode 1: orbital-energy-denominator preconditioned iteration with the same fixed point.

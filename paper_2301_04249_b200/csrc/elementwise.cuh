@@ -75,7 +75,8 @@ __global__ void k_unpack_t1(Dims d, const double* __restrict__ t1p, double* __re
 }
 
 // Tsc[(s,i,a)][pl][(s',m,e)] = t_{im}^{ae}
-__global__ void k_build_Tsc(Dims d, const double* __restrict__ t2p, double* __restrict__ Tsc)
+// Ts (optional, n1 x n1): Re + Im of every element, the left operand of the three-multiplication complex product (rtcc.cu step 9)
+__global__ void k_build_Tsc(Dims d, const double* __restrict__ t2p, double* __restrict__ Tsc, double* __restrict__ Ts)
 {
     const long long tot = (long long)d.n1 * d.n1;
     for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
@@ -90,11 +91,12 @@ __global__ void k_build_Tsc(Dims d, const double* __restrict__ t2p, double* __re
         else z = ab_amp(t2p, d, m, i, e, a);
         Tsc[(long long)r * 2 * d.n1 + c] = z.re;
         Tsc[(long long)r * 2 * d.n1 + d.n1 + c] = z.im;
+        if (Ts) Ts[x] = z.re + z.im;
     }
 }
 
 // T_AB[(i,B)][pl][(M,e)] = -tab[i,M,e,B]
-__global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __restrict__ TAB)
+__global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __restrict__ TAB, double* __restrict__ Ts)
 {
     const long long tot = (long long)d.nA * d.nB;
     for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
@@ -104,6 +106,20 @@ __global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __re
         c128 z = ab_amp(t2p, d, i, M, e, B);
         TAB[(long long)r * 2 * d.nB + c] = -z.re;
         TAB[(long long)r * 2 * d.nB + d.nB + c] = -z.im;
+        if (Ts) Ts[x] = -z.re - z.im;
+    }
+}
+
+// Right operand of the three-multiplication complex product: for a planar matrix W (rows x [Re cols | Im cols]) writes
+// Wd = Im - Re (rows x cols, dense) and replaces the Im plane by Re + Im.
+__global__ void k_r3m_W(long long rows, long long cols, double* __restrict__ W, double* __restrict__ Wd)
+{
+    const long long tot = rows * cols;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
+        const long long r = x / cols, c = x - r * cols;
+        const double re = W[r * 2 * cols + c], im = W[r * 2 * cols + cols + c];
+        Wd[x] = im - re;
+        W[r * 2 * cols + cols + c] = re + im;
     }
 }
 

@@ -21,6 +21,7 @@ using namespace rtcc;
 struct RtccOptions {
     int fused = 1, fused_fock = 1, graph = 1, prio = 1, tile = 0;
     int lean = -1, lean_slab_j = 0;              // lean: -1 automatic (when the standard layout does not fit), 0 never, 1 always
+    int ring3m = -1;                             // complex ring products by three real multiplications: -1 automatic, 0 never, 1 always
     LadderTune lad;
 };
 static RtccOptions g_opt;
@@ -44,6 +45,8 @@ struct rtcc_ctx {
     double *L[2]{}, *Lt[2]{}, *fockd[2]{}, *Fb[2]{}, *Ft[2]{}, *Kx[2]{}, *KxBA = nullptr;
     double *t1r = nullptr, *Tsc = nullptr, *Wsc = nullptr, *Zsc = nullptr;
     double *TAB = nullptr, *WBB = nullptr, *WAA = nullptr, *ZAB = nullptr, *ZBA = nullptr;
+    bool ring3m = false;                                          // T.W of the ring as three real products (standard layout only)
+    double *Ts_sc = nullptr, *Wd_sc = nullptr, *Ts_AB = nullptr, *Wd_BB = nullptr, *Wd_AA = nullptr;
     double *Nq = nullptr, *Mq = nullptr, *gam = nullptr, *r1buf = nullptr;
     double *Xab = nullptr, *tauab = nullptr, *Yab = nullptr, *Wooab = nullptr;
     double *LtA[2]{}, *LtB[2]{}, *Xt_ab = nullptr, *Xt_ss[2]{};   // tile-major ladder operands
@@ -145,6 +148,45 @@ void run(rtcc_ctx* c, TcGemm& g)
     int n = tcgemm_launch(g, c->S[c->si], cap, c->num_sms, &c->flops, c->opt.tile);
     c->launches += n;
 }
+// C (planar, row pitch ldc, Im plane at +pc) = alpha * (T W) + beta * C with three real products (see step 9 of the pipeline).
+//   Ts = Tr + Ti: element (m,k) at Ts[m * ts_m + k * ts_k];  T planar: (m,k) at T[m * t_m + k * t_k], Im plane at +pt
+//   W planar with pitch ldw: Re plane Wr, its Im plane (at +pw) already holds Wr + Wi;  Wd = Wi - Wr dense with pitch ldwd
+//   tr: the left operand is read transposed (m is the contiguous index)
+void cplx3m(rtcc_ctx* c, int M, int N, int K, const double* Ts, int tr, long long ts_m, long long ts_k,
+            const double* T, int tr2, long long t_m, long long t_k, long long pt,
+            const double* W, long long ldw, long long pw, const double* Wd, long long ldwd,
+            double* C, long long ldc, long long pc, double alpha, double beta)
+{
+    (void)tr2;
+    {   // k1 into both planes
+        TcGemm g = G0(M, N, K);
+        setA(g, 0, ts_m, 0, 0, ts_k, 0, tr ? 0 : 1);
+        setB(g, 0, ldw, 0, 1, 0, 1);
+        setC(g, 0, ldc, 0, 1);
+        ops_rr(g, Ts, W, C);
+        g.C2[0] = C + pc;
+        g.alpha = alpha; g.beta = beta;
+        run(c, g);
+    }
+    {   // Re -= k3 = Ti (Wr + Wi)
+        TcGemm g = G0(M, N, K);
+        setA(g, 0, t_m, 0, 0, t_k, 0, tr ? 0 : 1);
+        setB(g, 0, ldw, 0, 1, 0, 1);
+        setC(g, 0, ldc, 0, 1);
+        ops_rr(g, T + pt, W + pw, C);
+        g.alpha = -alpha; g.beta = 1.0;
+        run(c, g);
+    }
+    {   // Im += k2 = Tr (Wi - Wr)
+        TcGemm g = G0(M, N, K);
+        setA(g, 0, t_m, 0, 0, t_k, 0, tr ? 0 : 1);
+        setB(g, 0, ldwd, 0, 1, 0, 1);
+        setC(g, 0, ldc, 0, 1);
+        ops_rr(g, T, Wd, C + pc);
+        g.alpha = alpha; g.beta = 1.0;
+        run(c, g);
+    }
+}
 inline int nblk(long long n, int cap) { long long b = (n + 255) / 256; if (b < 1) b = 1; if (b > cap) b = cap; return (int)b; }
 #define EW(c, kern, n, ...) do { kern<<<nblk((n), (c)->num_sms * 16), 256, 0, (c)->S[(c)->si]>>>(__VA_ARGS__); (c)->launches++; } while (0)
 
@@ -177,8 +219,8 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     // ---- 1. unpack the packed spin blocks into the contraction layouts
     c->sec = 1;
     EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
-    EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc);
-    EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB);
+    EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc, c->ring3m ? c->Ts_sc : nullptr);
+    EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB, c->ring3m ? c->Ts_AB : nullptr);
     EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
     for (int s = 0; s < 2; ++s)
         if (d.po[s] > 0)
@@ -438,9 +480,15 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         if (s == 0 || d.n1a == 0) { WAITEV(1, 2); WAITEV(1, 7); }
         EW(c, k_add_Fd, (long long)o * v * v + (long long)o * o * v, o, v, n, c->Ft[s], o, c->Ft[s], o, c->Wsc, ld1, (long long)n1, off1, off1, 0, o);
     }
+    if (c->ring3m) EW(c, k_r3m_W, (long long)n1 * n1, (long long)n1, (long long)n1, c->Wsc, c->Wd_sc);
     LINK(1, 0, 3);
     BR(0);
-    {
+    if (c->ring3m) {
+        // (T W) with three real products instead of four (T = Tr + i Ti, W = Wr + i Wi):
+        //   k1 = (Tr + Ti) Wr,  k2 = Tr (Wi - Wr),  k3 = Ti (Wr + Wi);   Re(TW) = k1 - k3,  Im(TW) = k1 + k2
+        // Ts = Tr + Ti comes from the unpack kernel, k_r3m_W left Wr + Wi in W's Im plane and Wi - Wr in Wd.
+        cplx3m(c, n1, n1, n1, c->Ts_sc, 0, n1, 1, c->Tsc, 0, ld1, 1, n1, c->Wsc, ld1, n1, c->Wd_sc, n1, c->Zsc, ld1, n1, -1.0, 1.0);
+    } else {
         TcGemm g = G0(n1, n1, n1);
         setA(g, 0, ld1, 0, 0, 1, 0, 1);
         setB(g, 0, ld1, 0, 1, 0, 1);
@@ -478,7 +526,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         WAITEV(2, 2);
         WAITEV(2, 7);
         EW(c, k_add_Fd, (long long)ob * va * va + (long long)ob * ob * va, ob, va, n, c->Ft[1], ob, c->Ft[0], oa, c->WBB, lB, (long long)nB, 0LL, 0LL, 0, ob);
-        {
+        if (c->ring3m) {
+            EW(c, k_r3m_W, (long long)nB * nB, (long long)nB, (long long)nB, c->WBB, c->Wd_BB);
+            cplx3m(c, nA, nB, nB, c->Ts_AB, 0, nB, 1, c->TAB, 0, lB, 1, nB, c->WBB, lB, nB, c->Wd_BB, nB, c->ZAB, lB, nB, -1.0, 0.0);
+        } else {
             TcGemm g = G0(nA, nB, nB);
             setA(g, 0, lB, 0, 0, 1, 0, 1);
             setB(g, 0, lB, 0, 1, 0, 1);
@@ -506,7 +557,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             run(c, g);
         }
         EW(c, k_add_Fd, (long long)oa * vb * vb + (long long)oa * oa * vb, oa, vb, n, c->Ft[0], oa, c->Ft[1], ob, c->WAA, lA, (long long)nA, 0LL, 0LL, 0, oa);
-        {
+        if (c->ring3m) {                                   // left operand T_AB^T: k-fast = 0, rows stride 1
+            EW(c, k_r3m_W, (long long)nA * nA, (long long)nA, (long long)nA, c->WAA, c->Wd_AA);
+            cplx3m(c, nB, nA, nA, c->Ts_AB, 1, 1, nB, c->TAB, 1, 1, lB, nB, c->WAA, lA, nA, c->Wd_AA, nA, c->ZBA, lA, nA, -1.0, 0.0);
+        } else {
             TcGemm g = G0(nB, nA, nA);
             setA(g, 0, 1, 0, 0, lB, 0, 0);
             setB(g, 0, lA, 0, 1, 0, 1);
@@ -1294,7 +1348,10 @@ struct SizePlan {
 // Device memory of a context in doubles, in closed form (tested against rtcc_sizes).  standard: everything resident;
 // lean: persistent part + one arena shared by the ring phase (dressed vectors, same-spin pair-space blocks, one column
 // slab of W and Z, or the spin-flip W and Z) and the ladder phase (tile-major amplitudes and the ladder outputs).
-long long size_plan(const Dims& d, bool lean, int want_slab_j, SizePlan* out)
+// ring products large enough for the three-multiplication form (below this the two extra launches cost more than they save)
+inline bool ring3m_default(const Dims& d) { return d.n1 >= 1536; }
+
+long long size_plan(const Dims& d, bool lean, int want_slab_j, SizePlan* out, bool ring3m = false)
 {
     const long long n = d.n, nn = n * n, NQ = d.NQ, plane = NQ * nn, n1 = d.n1, nA = d.nA, nB = d.nB, oo = d.oo;
     const long long namp = d.n_t1 + d.n_t2;
@@ -1321,6 +1378,7 @@ long long size_plan(const Dims& d, bool lean, int want_slab_j, SizePlan* out)
     P += (32LL << 20) + 4 * 2 * namp;                                                    // GEMM workspace, gx, gr, t_cur, r_cur
     if (lean) P += oo * 2 * oo;                                                           // Voo
     else P += 3 * (2 * n1 * n1) + 3 * (2 * nA * nB) + 2 * nB * nB + 2 * nA * nA + 2 * ((long long)d.v[0] * d.v[1] * 2 * oo) + xt_ab + yab;
+    if (!lean && ring3m) P += 2 * n1 * n1 + nA * nB + nB * nB + nA * nA;                // Ts_sc, Wd_sc, Ts_AB, Wd_BB, Wd_AA
     sp.persistent = P;
     sp.xt_ab = xt_ab; sp.xt_ss[0] = xt_ss[0]; sp.xt_ss[1] = xt_ss[1];
     if (lean) {
@@ -1395,6 +1453,7 @@ int rtcc_set_default_option(const char* name, int value)
     else if (k == "ladder_cluster") { if (value < 0 || value > 16) return RTCC_EINVAL; g_opt.lad.force_cluster = value; }
     else if (k == "ladder_tiles") { if (value < 1 || value > LW_MAXC) return RTCC_EINVAL; g_opt.lad.max_tiles = value; }
     else if (k == "lean") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.lean = value; }
+    else if (k == "ring_3m") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.ring3m = value; }
     else if (k == "lean_slab") { if (value < 0) return RTCC_EINVAL; g_opt.lean_slab_j = value; }
     else if (k == "reset") g_opt = RtccOptions();
     else return RTCC_EINVAL;
@@ -1491,14 +1550,19 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         // lean or standard layout?
         {
             SizePlan sp;
-            const long long std_doubles = size_plan(d, false, 0, nullptr);
+            // three-multiplication ring products: worth two extra launches and 2 n1^2 + ... doubles once the products are large
+            bool r3m = c->opt.ring3m == 1 || (c->opt.ring3m == -1 && ring3m_default(d));
+            const long long std_doubles = size_plan(d, false, 0, nullptr, false);
+            const long long std3_doubles = size_plan(d, false, 0, nullptr, true);
             bool lean = c->opt.lean == 1;
             if (c->opt.lean == -1) {
                 size_t fr = 0, tot = 0;
                 CKC(cudaMemGetInfo(&fr, &tot));
+                if (r3m && (double)std3_doubles * 8.0 > 0.94 * (double)fr) r3m = false;
                 lean = (double)std_doubles * 8.0 > 0.94 * (double)fr;
             }
             c->lean = lean;
+            c->ring3m = r3m && !lean;
             if (lean) {
                 size_plan(d, true, c->opt.lean_slab_j, &sp);
                 c->arena_cap = sp.arena;
@@ -1567,6 +1631,13 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             DA(c->WAA, 2LL * d.nA * d.nA, "WAA");
             DA(c->ZAB, 2LL * d.nA * d.nB, "ZAB");
             DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
+            if (c->ring3m) {
+                DA(c->Ts_sc, (long long)n1 * n1, nullptr);
+                DA(c->Wd_sc, (long long)n1 * n1, nullptr);
+                DA(c->Ts_AB, (long long)d.nA * d.nB, nullptr);
+                DA(c->Wd_BB, (long long)d.nB * d.nB, nullptr);
+                DA(c->Wd_AA, (long long)d.nA * d.nA, nullptr);
+            }
         }
         DA(c->Mq, 2LL * NQ * n1, "Mq");
         if (c->fused_fock) {
@@ -1782,7 +1853,7 @@ int rtcc_problem_sizes(int oa, int ob, int va, int vb, int NQ, long long out[6])
     out[1] = d.n_t2;
     out[2] = (long long)oa * oa * va * va + (long long)ob * ob * vb * vb + (long long)oa * ob * va * vb;     // the paper's unpacked spin blocks
     out[3] = 2LL * NQ * d.n * d.n;
-    out[4] = 8 * size_plan(d, false, 0, nullptr);
+    out[4] = 8 * size_plan(d, false, 0, nullptr, ring3m_default(d));
     out[5] = 8 * size_plan(d, true, 0, nullptr);
     return RTCC_OK;
 }
@@ -1916,6 +1987,33 @@ int rtcc_load(rtcc_ctx* c, const char* path)
     CK(cudaStreamSynchronize(c->st));
     c->mode = h.mode; c->max_micro = h.max_micro; c->fixed_micro = h.fixed_micro; c->tol = h.tol;
     c->time = h.time; c->C[0] = h.C[0]; c->C[1] = h.C[1]; c->E[0] = h.E[0]; c->E[1] = h.E[1];
+    c->state_valid = true;
+    return RTCC_OK;
+}
+
+int rtcc_get_state(const rtcc_ctx* cc, double* t1, double* t2, double* r1, double* r2, double scal[5])
+{
+    rtcc_ctx* c = const_cast<rtcc_ctx*>(cc);
+    if (!c || !t1 || !t2 || !r1 || !r2 || !scal) return RTCC_EINVAL;
+    { int rc0 = ensure_state(c); if (rc0) return rc0; }
+    const Dims& d = c->d;
+    if (copy_out(c, t1, c->t_cur, 2 * d.n_t1) || copy_out(c, t2, c->t_cur + 2 * d.n_t1, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (copy_out(c, r1, c->r_cur, 2 * d.n_t1) || copy_out(c, r2, c->r_cur + 2 * d.n_t1, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (cudaStreamSynchronize(c->st) != cudaSuccess) return RTCC_ECUDA;
+    scal[0] = c->time; scal[1] = c->C[0]; scal[2] = c->C[1]; scal[3] = c->E[0]; scal[4] = c->E[1];
+    return RTCC_OK;
+}
+
+int rtcc_set_state(rtcc_ctx* c, const double* t1, const double* t2, const double* r1, const double* r2, const double scal[5])
+{
+    if (!c || !t1 || !t2 || !r1 || !r2 || !scal) return RTCC_EINVAL;
+    for (int i = 0; i < 5; ++i) if (!std::isfinite(scal[i])) return RTCC_EINVAL;
+    const Dims& d = c->d;
+    // no residual evaluation: R(T(tau)) and E(tau) are part of the state the caller hands back
+    if (copy_in(c, c->t_cur, t1, 2 * d.n_t1) || copy_in(c, c->t_cur + 2 * d.n_t1, t2, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (copy_in(c, c->r_cur, r1, 2 * d.n_t1) || copy_in(c, c->r_cur + 2 * d.n_t1, r2, 2 * d.n_t2)) return RTCC_ECUDA;
+    if (c->flags & RTCC_HOST_PTRS) CK(cudaStreamSynchronize(c->st));      // the caller may reuse its host arrays on return
+    c->time = scal[0]; c->C[0] = scal[1]; c->C[1] = scal[2]; c->E[0] = scal[3]; c->E[1] = scal[4];
     c->state_valid = true;
     return RTCC_OK;
 }
@@ -2057,16 +2155,22 @@ int rtcc_build_fock(int n, int NQ, const double* L, const double* eps, int cs, i
     const long long nn = (long long)n * n, nL = 2LL * NQ * nn;
     const double *dL = L, *de = eps; double* df = fock;
     double* buf = nullptr;
+    cudaError_t e = cudaSuccess;
     if (flags & RTCC_HOST_PTRS) {
         if (cudaMalloc(&buf, (size_t)(nL + 2 * n + 2 * nn) * 8) != cudaSuccess) { cudaGetLastError(); return RTCC_ENOMEM; }
-        cudaMemcpyAsync(buf, L, (size_t)nL * 8, cudaMemcpyHostToDevice, st);
-        cudaMemcpyAsync(buf + nL, eps, (size_t)2 * n * 8, cudaMemcpyHostToDevice, st);
+        e = cudaMemcpyAsync(buf, L, (size_t)nL * 8, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(buf + nL, eps, (size_t)2 * n * 8, cudaMemcpyHostToDevice, st);
         dL = buf; de = buf + nL; df = buf + nL + 2 * n;
     }
-    k_build_fock<<<nblk(2 * nn, 148 * 8), 256, 0, st>>>(n, NQ, dL, de, cs, ci, df);
-    if (flags & RTCC_HOST_PTRS) cudaMemcpyAsync(fock, df, (size_t)2 * nn * 8, cudaMemcpyDeviceToHost, st);
-    cudaError_t e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) {
+        k_build_fock<<<nblk(2 * nn, 148 * 8), 256, 0, st>>>(n, NQ, dL, de, cs, ci, df);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess && (flags & RTCC_HOST_PTRS)) e = cudaMemcpyAsync(fock, df, (size_t)2 * nn * 8, cudaMemcpyDeviceToHost, st);
+    const cudaError_t es = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = es;
     if (buf) cudaFree(buf);
+    if (e != cudaSuccess) cudaGetLastError();
     return e == cudaSuccess ? RTCC_OK : RTCC_ECUDA;
 }
 
@@ -2096,7 +2200,7 @@ int rtcc_fp64_peak(double* tflops)
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return RTCC_ECUDA;
     double* buf = nullptr;
     const int grid = sms * 2, iters = 4000;
-    if (cudaMalloc(&buf, (size_t)grid * 256 * 8) != cudaSuccess) return RTCC_ENOMEM;
+    if (cudaMalloc(&buf, (size_t)grid * 256 * 8) != cudaSuccess) { cudaGetLastError(); return RTCC_ENOMEM; }
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     float best = 1e30f;

@@ -30,6 +30,7 @@ struct TcGemm {
     const double* A[TG_MAXB][2];
     const double* B[TG_MAXB][2];
     double* C[TG_MAXB];
+    double* C2[TG_MAXB];                     // optional second output with the strides of C (the same product lands in both)
     signed char nphase[TG_MAXB], s0[TG_MAXB], s1[TG_MAXB];
     int nsb;                                 // strided batches
     long long sbA, sbB, sbC;
@@ -288,6 +289,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
         return;
     }
     double* C = g.C[db] + sb * g.sbC;
+    double* C2 = g.C2[db] ? g.C2[db] + sb * g.sbC : nullptr;
     const double al = g.alpha * sgn, be = g.beta;
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
@@ -300,8 +302,14 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
             for (int e = 0; e < 2; ++e) {
                 int n = n0 + wn0 + 8 * j + 2 * lc + e;
                 if (n < g.N) {
-                    double* p = C + mo + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+                    const long long co = mo + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+                    double* p = C + co;
                     double v = al * acc[i][j][e];
+                    if (C2) {
+                        double v2 = v;
+                        if (be != 0.0) v2 += be * C2[co];
+                        C2[co] = v2;
+                    }
                     if (be != 0.0) v += be * *p;
                     *p = v;
                 }
@@ -323,8 +331,14 @@ __global__ void tcgemm_splitk_reduce(const TcGemm g)
         const double* W = g.ws + (long long)bt * g.ksplit * MN + r;
         double s = 0.0;
         for (int k = 0; k < g.ksplit; ++k) s += W[k * MN];
-        double* p = g.C[db] + sb * g.sbC + (g.cm_table ? g.cm_table[m] : idx2(m, g.Mlo, g.cm_hi, g.cm_lo)) + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+        const long long co = sb * g.sbC + (g.cm_table ? g.cm_table[m] : idx2(m, g.Mlo, g.cm_hi, g.cm_lo)) + idx2(n, g.Nlo, g.cn_hi, g.cn_lo);
+        double* p = g.C[db] + co;
         double v = g.alpha * s;
+        if (g.C2[db]) {
+            double v2 = v;
+            if (g.beta != 0.0) v2 += g.beta * g.C2[db][co];
+            g.C2[db][co] = v2;
+        }
         if (g.beta != 0.0) v += g.beta * *p;
         *p = v;
     }

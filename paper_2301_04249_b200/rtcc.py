@@ -23,6 +23,7 @@ SYMBOLS = [
     "rtcc_counters", "rtcc_reset_counters", "rtcc_set_timing", "rtcc_ladder_timing", "rtcc_fp64_peak",
     "rtcc_debug_buffer", "rtcc_debug_gemm", "rtcc_last_cuda_error", "rtcc_strerror", "rtcc_build_fock", "rtcc_spectral_function",
     "rtcc_set_default_option", "rtcc_ladder_plan", "rtcc_ladder_occupancy", "rtcc_save", "rtcc_load", "rtcc_problem_sizes",
+    "rtcc_get_state", "rtcc_set_state",
 ]
 
 
@@ -68,6 +69,8 @@ def load():
         lib.rtcc_problem_sizes.argtypes = [i, i, i, i, i, P(ll)]
         lib.rtcc_save.argtypes = [vp, ctypes.c_char_p]
         lib.rtcc_load.argtypes = [vp, ctypes.c_char_p]
+        lib.rtcc_get_state.argtypes = [vp, vp, vp, vp, vp, P(d)]
+        lib.rtcc_set_state.argtypes = [vp, vp, vp, vp, vp, P(d)]
         lib.rtcc_last_cuda_error.argtypes = [vp]
         lib.rtcc_strerror.argtypes = [i]; lib.rtcc_strerror.restype = ctypes.c_char_p
         _lib = lib
@@ -247,6 +250,20 @@ class Rtcc:
 
     def load(self, path: str):
         self._ck(self._lib.rtcc_load(self._h, os.fsencode(path)), "rtcc_load")
+
+    def get_state(self, out=None):
+        """(t1, t2, r1, r2, tau, C, E): the propagation state T(tau), R(T(tau)) and its scalars, through memory.
+        `out` = (t1, t2, r1, r2) arrays to fill instead of new ones."""
+        t1, t2, r1, r2 = out if out is not None else (self._new(self.n_t1), self._new(self.n_t2), self._new(self.n_t1), self._new(self.n_t2))
+        sc = (ctypes.c_double * 5)()
+        self._ck(self._lib.rtcc_get_state(self._h, _ptr(t1), _ptr(t2), _ptr(r1), _ptr(r2), sc), "rtcc_get_state")
+        return t1, t2, r1, r2, sc[0], complex(sc[1], sc[2]), complex(sc[3], sc[4])
+
+    def set_state(self, t1, t2, r1, r2, time, C, E):
+        """Install a state taken with get_state (no residual evaluation)."""
+        t1 = self._chk(t1, self.n_t1); t2 = self._chk(t2, self.n_t2); r1 = self._chk(r1, self.n_t1); r2 = self._chk(r2, self.n_t2)
+        sc = (ctypes.c_double * 5)(float(time), complex(C).real, complex(C).imag, complex(E).real, complex(E).imag)
+        self._ck(self._lib.rtcc_set_state(self._h, _ptr(t1), _ptr(t2), _ptr(r1), _ptr(r2), sc), "rtcc_set_state")
 
     def set_solver(self, mode=0, tol=1e-4, max_micro=200, fixed_micro=0):
         self._ck(self._lib.rtcc_set_solver(self._h, mode, tol, max_micro, fixed_micro), "rtcc_set_solver")

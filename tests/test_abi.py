@@ -82,6 +82,6 @@ def test_memory_budget_of_the_baseline_configs(lib):
         if name == "largest":
             assert ps["bytes_standard"] > 300 * GB and ps["bytes_lean"] < 175 * GB
         else:
-            assert ps["bytes_standard"] < 150 * GB
+            assert ps["bytes_standard"] < 160 * GB            # Large: 150 GB incl. the 18 GB of the three-multiplication ring operands
     with pytest.raises(rtcc.RtccError):
         rtcc.problem_sizes(1, 1, 2, 3, 4)

@@ -118,6 +118,27 @@ def test_wide_ladder_cluster_shapes(rtcc, opts):
 _WIDE_REF = {}
 
 
+@pytest.mark.parametrize("shape", [(3, 4, 13, 12, 48), (2, 0, 3, 5, 4), (0, 2, 5, 3, 4), (1, 2, 2, 1, 3), (9, 8, 10, 11, 20), (5, 4, 18, 19, 37)])
+@pytest.mark.parametrize("fused", [1, 0])
+def test_ring_three_multiplication_products(rtcc, shape, fused):
+    """The ring's complex x complex products T.W (spin-conserving sector and both spin-flip products, one with the left operand
+    transposed) as three real multiplications -- the form the library picks by itself from a pair-space dimension of 1536 (Mid,
+    Large) -- forced on sizes the full oracle checks element by element, incl. shapes with an empty spin-flip sector."""
+    oa, ob, va, vb, K = shape
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=300 + sum(shape))
+    d = orc.Dims(oa, ob, va, vb, K)
+    rng = np.random.default_rng(11)
+    t1 = 0.1 * (rng.standard_normal(d.n_t1) + 1j * rng.standard_normal(d.n_t1))
+    t2 = 0.1 * (rng.standard_normal(d.n_t2) + 1j * rng.standard_normal(d.n_t2))
+    try:
+        rtcc.set_default_option("ring_3m", 1)
+        rtcc.set_default_option("fused", fused)
+        rtcc.set_default_option("fused_fock", fused)
+        check_residual(rtcc, oa, ob, va, vb, K, L, fock, t1, t2)
+    finally:
+        rtcc.set_default_option("reset")
+
+
 def test_residual_tiny_config_literal_generator(rtcc):
     """BASELINE.json config 1 (Tiny): literal generator, seeded N(0,1e-3) complex amplitudes and t = 0."""
     cfg = inputs.CONFIGS["tiny"]
@@ -343,6 +364,43 @@ def test_checkpoint_restart_continues_bit_identically_and_matches_oracle(rtcc, t
         c.close()
 
 
+@pytest.mark.parametrize("device", [False, True])
+def test_state_through_memory_continues_bit_identically_and_matches_oracle(rtcc, device):
+    """rtcc_get_state / rtcc_set_state (the checkpoint of PAPER.md:135 through memory, the call bench.py's e2e leg makes every
+    step): a second context continued from the state of the first equals the uninterrupted run bit for bit and the oracle
+    propagated straight through within 1e-8 on C; host-pointer and device-pointer contexts."""
+    import torch
+    cfg = inputs.CONFIGS["tiny"]
+    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=0.2)
+    prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+    po = orc.Propagator(prob, mode=0, tol=1e-12, max_micro=200)
+    mk = (lambda: rtcc.Rtcc(oa, ob, va, vb, K, torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda())) if device else \
+         (lambda: rtcc.Rtcc(oa, ob, va, vb, K, L, fock))
+    straight, first, second = mk(), mk(), mk()
+    for c in (straight, first, second):
+        c.set_solver(mode=0, tol=1e-12, max_micro=200)
+    for _ in range(5):
+        po.step(cfg.dt); straight.step(cfg.dt); first.step(cfg.dt)
+    st = first.get_state()
+    assert st[4] == straight.time and (st[5], st[6]) == straight.cumulant()
+    first.close()
+    second.set_state(*st)
+    for _ in range(5):                              # every step through memory, as the e2e leg does
+        po.step(cfg.dt); straight.step(cfg.dt); second.step(cfg.dt)
+        st = second.get_state(out=st[:4])
+        second.set_state(*st)
+    assert second.cumulant() == straight.cumulant() and second.time == straight.time
+    a, b = second.get_amplitudes(), straight.get_amplitudes()
+    eq = (lambda x, y: bool(torch.equal(x, y))) if device else np.array_equal
+    assert eq(a[0], b[0]) and eq(a[1], b[1])
+    C, E = second.cumulant()
+    assert abs(C - po.C) <= CTOL * abs(po.C) and abs(E - po.E) <= CTOL * abs(po.E)
+    with pytest.raises(rtcc.RtccError) as ei:
+        second.set_state(st[0], st[1], st[2], st[3], float("nan"), st[5], st[6])
+    assert ei.value.code == -1 and second.cumulant() == straight.cumulant()
+    straight.close(); second.close()
+
+
 def test_contraction_primitive_against_matmul(rtcc):
     rng = np.random.default_rng(0)
     # the last shape is large enough (two full waves of 128x128 tiles) to run the big-tile kernel
@@ -450,39 +508,3 @@ def test_spectral_function_matches_oracle(rtcc):
     G, A = rtcc.spectral_function(Cs, cfg.dt, -20.0, -0.25, 0.2, om)
     assert np.abs(G - Go).max() <= 1e-12
     assert np.abs(A - Ao).max() <= 1e-10 * np.abs(Ao).max()
-
-
-@pytest.mark.skipif(not __import__("os").environ.get("RTCC_RUN_MID"), reason="several minutes and ~12 GB of host memory: set RTCC_RUN_MID=1")
-def test_residual_mid_config_sampled(rtcc):
-    """BASELINE.json config 3 (Mid: o=24, v=200, n_chol=900) at full size: the general tcgemm path (no fused small kernels),
-    128x128 tiles at scale and the cluster ladder (clusters of 9 / 4 / 5) against the sampled-element oracle."""
-    import torch
-    from oracle.sampled import SampledOracle
-    cfg = inputs.CONFIGS["mid"]
-    oa, ob, va, vb, K, L, fock = inputs.make_problem(cfg, sigma=inputs.stabilised_sigma(cfg))
-    t1, t2 = inputs.random_amplitudes(cfg, std=2e-2)
-    ctx = rtcc.Rtcc(oa, ob, va, vb, K, torch.from_numpy(L).cuda(), torch.from_numpy(fock).cuda())
-    r1d, r2d = ctx.residual(torch.from_numpy(t1).cuda(), torch.from_numpy(t2).cuda())
-    r1, r2 = r1d.cpu().numpy(), r2d.cpu().numpy()
-    E = ctx.residual_energy()
-    ctx.close()
-    torch.cuda.empty_cache()
-    scale = max(np.abs(r1).max(), np.abs(r2).max())
-    so = SampledOracle(oa, ob, va, vb, K, L, fock, t1, t2)
-    d = so.d
-    naa = orc.npair(oa) * orc.npair(va)
-    nbb = orc.npair(ob) * orc.npair(vb)
-    rng = np.random.default_rng(4250)
-    picks = [0, naa - 1, naa, naa + nbb - 1, naa + nbb, d.n_t2 - 1]
-    picks += list(rng.integers(0, naa, 4)) + list(naa + rng.integers(0, nbb, 4)) + list(naa + nbb + rng.integers(0, d.n_t2 - naa - nbb, 8))
-    worst = 0.0
-    for k in picks:
-        i, j, a, b = so.so_of_packed_t2(int(k))
-        worst = max(worst, abs(so.r2(i, j, a, b) - r2[int(k)]))
-    for k in list(rng.integers(0, d.n_t1, 6)) + [0, d.n_t1 - 1]:
-        i, a = so.so_of_packed_t1(int(k))
-        worst = max(worst, abs(so.r1(i, a) - r1[int(k)]))
-    print("mid sampled parity: worst", worst, "scale", scale)
-    assert worst <= RTOL * scale, (worst, scale)
-    Eo = so.energy()
-    assert abs(E - Eo) <= RTOL * max(scale, abs(Eo))
