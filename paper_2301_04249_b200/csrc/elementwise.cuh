@@ -74,42 +74,6 @@ __global__ void k_unpack_t1(Dims d, const double* __restrict__ t1p, double* __re
     }
 }
 
-// Tsc[(s,i,a)][pl][(s',m,e)] = t_{im}^{ae}
-// Ts (optional, n1 x n1): Re + Im of every element, the left operand of the three-multiplication complex product (rtcc.cu step 9)
-__global__ void k_build_Tsc(Dims d, const double* __restrict__ t2p, double* __restrict__ Tsc, double* __restrict__ Ts)
-{
-    const long long tot = (long long)d.n1 * d.n1;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
-        int r = (int)(x / d.n1), c = (int)(x - (long long)r * d.n1);
-        int sr = r >= d.n1a, sc = c >= d.n1a;
-        int rr = sr ? r - d.n1a : r, cc = sc ? c - d.n1a : c;
-        int i = rr / d.v[sr], a = rr - i * d.v[sr];
-        int m = cc / d.v[sc], e = cc - m * d.v[sc];
-        c128 z;
-        if (sr == sc) z = ss_amp(t2p, d.off_t2[sr], d.pv[sr], i, m, a, e);
-        else if (sr == 0) z = ab_amp(t2p, d, i, m, a, e);
-        else z = ab_amp(t2p, d, m, i, e, a);
-        Tsc[(long long)r * 2 * d.n1 + c] = z.re;
-        Tsc[(long long)r * 2 * d.n1 + d.n1 + c] = z.im;
-        if (Ts) Ts[x] = z.re + z.im;
-    }
-}
-
-// T_AB[(i,B)][pl][(M,e)] = -tab[i,M,e,B]
-__global__ void k_build_TAB(Dims d, const double* __restrict__ t2p, double* __restrict__ TAB, double* __restrict__ Ts)
-{
-    const long long tot = (long long)d.nA * d.nB;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
-        int r = (int)(x / d.nB), c = (int)(x - (long long)r * d.nB);
-        int i = r / d.v[1], B = r - i * d.v[1];
-        int M = c / d.v[0], e = c - M * d.v[0];
-        c128 z = ab_amp(t2p, d, i, M, e, B);
-        TAB[(long long)r * 2 * d.nB + c] = -z.re;
-        TAB[(long long)r * 2 * d.nB + d.nB + c] = -z.im;
-        if (Ts) Ts[x] = -z.re - z.im;
-    }
-}
-
 // Right operand of the three-multiplication complex product: for a planar matrix W (rows x [Re cols | Im cols]) writes
 // Wd = Im - Re (rows x cols, dense) and replaces the Im plane by Re + Im.
 __global__ void k_r3m_W(long long rows, long long cols, double* __restrict__ W, double* __restrict__ Wd)
@@ -120,6 +84,116 @@ __global__ void k_r3m_W(long long rows, long long cols, double* __restrict__ W, 
         const double re = W[r * 2 * cols + c], im = W[r * 2 * cols + cols + c];
         Wd[x] = im - re;
         W[r * 2 * cols + cols + c] = re + im;
+    }
+}
+
+// Tiled unpacking of the pair-space amplitude matrices (north_star: "coalesced ... shared-memory staging").  Every packed
+// amplitude is read ONCE, as a 16-byte complex element with the packed layout's fastest index across the threads, and written
+// to all the places the pair-space matrices hold it -- directly where the destination's fastest index is the source's, through
+// a 32 x 33 shared-memory tile (transposed) where it is the other one.  T_sc and T_AB are symmetric / share their elements:
+//   alpha-beta amplitude t = tab[i,M,a,E]:  Tsc[(a i a),(b M E)] = Tsc[(b M E),(a i a)] = t,   T_AB[(i,E),(M,a)] = -t
+//   same-spin amplitude t = t_{i<m}^{a<e}:  T[(i,a),(m,e)] = T[(m,e),(i,a)] = t,  T[(i,e),(m,a)] = T[(m,a),(i,e)] = -t
+// (elements with i == m or a == e are zero: the buffers are cleared once at creation and those places never written).
+// Ts / TsAB (optional): Re + Im of every element, the left operand of the three-multiplication complex product.
+constexpr int UP_T = 32;
+__global__ void __launch_bounds__(256) k_unpack_ab(Dims d, const double* __restrict__ t2p, double* __restrict__ Tsc, double* __restrict__ TAB,
+                                                   double* __restrict__ Ts, double* __restrict__ TsAB)
+{
+    __shared__ double sre[UP_T][UP_T + 1], sim[UP_T][UP_T + 1];
+    const int oa = d.o[0], ob = d.o[1], va = d.v[0], vb = d.v[1];
+    const int nAt = (va + UP_T - 1) / UP_T, nEt = (vb + UP_T - 1) / UP_T;
+    const long long nitem = (long long)oa * ob * nAt * nEt;
+    const long long n1 = d.n1, ld = 2 * n1, nB = d.nB;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(t2p) + d.off_t2[2];
+    for (long long it = blockIdx.x; it < nitem; it += gridDim.x) {
+        long long k = it;
+        const int E0 = (int)(k % nEt) * UP_T; k /= nEt;
+        const int a0 = (int)(k % nAt) * UP_T; k /= nAt;
+        const int M = (int)(k % ob), i = (int)(k / ob);
+        const long long base = ((long long)i * ob + M) * va;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int a = a0 + ty + 8 * q, E = E0 + tx;
+            double2 z = make_double2(0.0, 0.0);
+            if (a < va && E < vb) {
+                z = src[(base + a) * vb + E];
+                const long long r = (long long)i * va + a, c = d.n1a + (long long)M * vb + E;
+                Tsc[r * ld + c] = z.x;
+                Tsc[r * ld + n1 + c] = z.y;
+                if (Ts) Ts[r * n1 + c] = z.x + z.y;
+            }
+            sre[ty + 8 * q][tx] = z.x; sim[ty + 8 * q][tx] = z.y;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int E = E0 + ty + 8 * q, a = a0 + tx;
+            if (a < va && E < vb) {
+                const double re = sre[tx][ty + 8 * q], im = sim[tx][ty + 8 * q];
+                const long long r = d.n1a + (long long)M * vb + E, c = (long long)i * va + a;
+                Tsc[r * ld + c] = re;
+                Tsc[r * ld + n1 + c] = im;
+                if (Ts) Ts[r * n1 + c] = re + im;
+                const long long rA = (long long)i * vb + E, cA = (long long)M * va + a;
+                TAB[rA * 2 * nB + cA] = -re;
+                TAB[rA * 2 * nB + nB + cA] = -im;
+                if (TsAB) TsAB[rA * nB + cA] = -re - im;
+            }
+        }
+    }
+}
+__global__ void __launch_bounds__(256) k_unpack_ss(Dims d, int s, const int2* __restrict__ opairs, const double* __restrict__ t2p,
+                                                   double* __restrict__ Tsc, double* __restrict__ Ts)
+{
+    __shared__ double sre[UP_T][UP_T + 1], sim[UP_T][UP_T + 1];
+    const int v = d.v[s], po = d.po[s], pv = d.pv[s];
+    const int nT = (v + UP_T - 1) / UP_T, ntri = nT * (nT + 1) / 2;
+    const long long nitem = (long long)po * ntri;
+    const long long n1 = d.n1, ld = 2 * n1, off = s ? d.n1a : 0;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(t2p) + d.off_t2[s];
+    for (long long it = blockIdx.x; it < nitem; it += gridDim.x) {
+        const int pim = (int)(it / ntri); int tt = (int)(it - (long long)pim * ntri);
+        int et = 0;                                          // tile pair (at <= et) from the triangular index
+        while ((et + 1) * (et + 2) / 2 <= tt) ++et;
+        const int at = tt - et * (et + 1) / 2;
+        const int a0 = at * UP_T, e0 = et * UP_T;
+        const int2 im_ = opairs[pim];
+        const long long ri = off + (long long)im_.x * v, rm = off + (long long)im_.y * v;    // first row / column of (i,.) and (m,.)
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int e = e0 + ty + 8 * q, a = a0 + tx;
+            double2 z = make_double2(0.0, 0.0);
+            if (a < e && e < v) {
+                z = src[(long long)pim * pv + pair_index(a, e)];
+                // destinations whose fastest index is a:  T[(i,e),(m,a)] = -t,  T[(m,e),(i,a)] = +t
+                long long r = ri + e, c = rm + a;
+                Tsc[r * ld + c] = -z.x; Tsc[r * ld + n1 + c] = -z.y;
+                if (Ts) Ts[r * n1 + c] = -z.x - z.y;
+                r = rm + e; c = ri + a;
+                Tsc[r * ld + c] = z.x; Tsc[r * ld + n1 + c] = z.y;
+                if (Ts) Ts[r * n1 + c] = z.x + z.y;
+            }
+            sre[ty + 8 * q][tx] = z.x; sim[ty + 8 * q][tx] = z.y;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int a = a0 + ty + 8 * q, e = e0 + tx;
+            if (a < e && e < v) {
+                const double re = sre[tx][ty + 8 * q], im = sim[tx][ty + 8 * q];
+                // destinations whose fastest index is e:  T[(i,a),(m,e)] = +t,  T[(m,a),(i,e)] = -t
+                long long r = ri + a, c = rm + e;
+                Tsc[r * ld + c] = re; Tsc[r * ld + n1 + c] = im;
+                if (Ts) Ts[r * n1 + c] = re + im;
+                r = rm + a; c = ri + e;
+                Tsc[r * ld + c] = -re; Tsc[r * ld + n1 + c] = -im;
+                if (Ts) Ts[r * n1 + c] = -re - im;
+            }
+        }
     }
 }
 
@@ -297,6 +371,9 @@ __global__ void k_assemble(Dims d, AsmArgs A)
 // contiguity class with the matching index fastest across the threads (full sectors), accumulates in shared memory, and
 // writes the packed output with its own fastest index.  Summation order per element is fixed: bit-reproducible.
 constexpr int AS_TJ = 8, AS_TA = 16, AS_TB = 16, AS_PB = AS_TB + 1;
+// Each sweep first issues all of a thread's loads (AS_NIT independent 8-byte loads per source, kept in registers), then
+// accumulates: the loads of a sweep are in flight together instead of one dependent round trip per element.
+constexpr int AS_NIT = 2 * AS_TJ * AS_TA * AS_TB / 256;
 // alpha-beta block: r2[i,J,a,B] = Zsc[ia,JB] + Zsc[JB,ia] - Z_AB[iB,Ja] - Z_BA[Ja,iB] + Y[(a,B)][(i,J)]
 __global__ void __launch_bounds__(256) k_assemble_ab(Dims d, AsmArgs A)
 {
@@ -305,41 +382,72 @@ __global__ void __launch_bounds__(256) k_assemble_ab(Dims d, AsmArgs A)
     const int nJt = (ob + AS_TJ - 1) / AS_TJ, nAt = (va + AS_TA - 1) / AS_TA, nBt = (vb + AS_TB - 1) / AS_TB;
     const long long ntile = (long long)oa * nJt * nAt * nBt;
     const long long ld = 2LL * d.n1, nss = (long long)d.po[0] * d.pv[0] + (long long)d.po[1] * d.pv[1];
+    const long long n1 = d.n1, nA = d.nA, nB = d.nB, oo = d.oo;
     const int tid = threadIdx.x;
+    const double* __restrict__ Zsc = A.Zsc;
+    const double* __restrict__ ZAB = A.ZAB;
+    const double* __restrict__ ZBA = A.ZBA;
+    const double* __restrict__ Yab = A.Yab;
     for (long long t = blockIdx.x; t < ntile; t += gridDim.x) {
         long long k = t;
         const int B0 = (int)(k % nBt) * AS_TB; k /= nBt;
         const int a0 = (int)(k % nAt) * AS_TA; k /= nAt;
         const int J0 = (int)(k % nJt) * AS_TJ; const int i = (int)(k / nJt);
+        double val[AS_NIT];
         __syncthreads();
         // class "B fastest": Zsc[ia,JB] - Z_BA[Ja,iB]
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int b = x % AS_TB, a = (x / AS_TB) % AS_TA, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int B = B0 + b, aa = a0 + a, J = J0 + j;
             double v = 0.0;
             if (B < vb && aa < va && J < ob) {
                 const long long ia = (long long)i * va + aa, JB = d.n1a + (long long)J * vb + B, iB = (long long)i * vb + B, Ja = (long long)J * va + aa;
-                v = A.Zsc[ia * ld + pl * (long long)d.n1 + JB] - A.ZBA[Ja * 2 * d.nA + pl * (long long)d.nA + iB];
+                v = Zsc[ia * ld + pl * n1 + JB] - ZBA[Ja * 2 * nA + pl * nA + iB];
             }
-            acc[pl][j][a][b] = v;
+            val[it] = v;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][(x / (AS_TB * AS_TA)) % AS_TJ][(x / AS_TB) % AS_TA][x % AS_TB] = val[it];
         }
         __syncthreads();
         // class "a fastest": Zsc[JB,ia] - Z_AB[iB,Ja]
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int a = x % AS_TA, b = (x / AS_TA) % AS_TB, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            double v = 0.0;
             if (B < vb && aa < va && J < ob) {
                 const long long ia = (long long)i * va + aa, JB = d.n1a + (long long)J * vb + B, iB = (long long)i * vb + B, Ja = (long long)J * va + aa;
-                acc[pl][j][a][b] += A.Zsc[JB * ld + pl * (long long)d.n1 + ia] - A.ZAB[iB * 2 * d.nB + pl * (long long)d.nB + Ja];
+                v = Zsc[JB * ld + pl * n1 + ia] - ZAB[iB * 2 * nB + pl * nB + Ja];
             }
+            val[it] = v;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][(x / (AS_TB * AS_TA)) % AS_TJ][x % AS_TA][(x / AS_TA) % AS_TB] += val[it];
         }
         __syncthreads();
         // class "J fastest": ladder output Y[(a,B)][(i,J)]
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int j = x % AS_TJ, b = (x / AS_TJ) % AS_TB, a = (x / (AS_TJ * AS_TB)) % AS_TA, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int B = B0 + b, aa = a0 + a, J = J0 + j;
+            double v = 0.0;
             if (B < vb && aa < va && J < ob)
-                acc[pl][j][a][b] += A.Yab[((long long)(oa + aa) * d.n + ob + B) * 2 * d.oo + pl * (long long)d.oo + (long long)i * ob + J];
+                v = Yab[((long long)(oa + aa) * d.n + ob + B) * 2 * oo + pl * oo + (long long)i * ob + J];
+            val[it] = v;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][x % AS_TJ][(x / (AS_TJ * AS_TB)) % AS_TA][(x / AS_TJ) % AS_TB] += val[it];
         }
         __syncthreads();
         // packed output, B fastest, (re, im) interleaved
@@ -360,48 +468,76 @@ __global__ void __launch_bounds__(256) k_assemble_ss(Dims d, int s, AsmArgs A)
     const int o = d.o[s], v = d.v[s], po = d.po[s], pv = d.pv[s];
     const int nPt = (po + AS_TJ - 1) / AS_TJ, nAt = (v + AS_TA - 1) / AS_TA, nBt = (v + AS_TB - 1) / AS_TB;
     const long long ntile = (long long)nPt * nAt * nBt;
-    const long long ld = 2LL * d.n1, off = s ? d.n1a : 0, obase = s ? (long long)d.po[0] * d.pv[0] : 0;
+    const long long ld = 2LL * d.n1, n1 = d.n1, off = s ? d.n1a : 0, obase = s ? (long long)d.po[0] * d.pv[0] : 0;
     const int tid = threadIdx.x;
-    const int2* op = A.opairs[s];
+    const int2* __restrict__ op = A.opairs[s];
+    const double* __restrict__ Zsc = A.Zsc;
+    const double* __restrict__ Yss = A.Yss[s];
+    const double* __restrict__ Zv = A.Zv[s];
     for (long long t = blockIdx.x; t < ntile; t += gridDim.x) {
         long long k = t;
         const int b0 = (int)(k % nBt) * AS_TB; k /= nBt;
         const int a0 = (int)(k % nAt) * AS_TA; const int p0 = (int)(k / nAt) * AS_TJ;
         if (a0 >= b0 + AS_TB) continue;                    // no a < b in this tile (block-uniform)
+        double val[AS_NIT];
         __syncthreads();
         // class "b fastest": Z[ia,jb] - Z[ja,ib]
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int b = x % AS_TB, a = (x / AS_TB) % AS_TA, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
-            double val = 0.0;
+            double w = 0.0;
             if (aa < bb && bb < v && pij < po) {
                 const int2 ij = op[pij];
                 const long long ia = off + (long long)ij.x * v + aa, jb = off + (long long)ij.y * v + bb, ja = off + (long long)ij.y * v + aa, ib = off + (long long)ij.x * v + bb;
-                val = A.Zsc[ia * ld + pl * (long long)d.n1 + jb] - A.Zsc[ja * ld + pl * (long long)d.n1 + ib];
+                w = Zsc[ia * ld + pl * n1 + jb] - Zsc[ja * ld + pl * n1 + ib];
             }
-            acc[pl][j][a][b] = val;
+            val[it] = w;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][(x / (AS_TB * AS_TA)) % AS_TJ][(x / AS_TB) % AS_TA][x % AS_TB] = val[it];
         }
         __syncthreads();
         // class "a fastest": - Z[ib,ja] + Z[jb,ia]
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int a = x % AS_TA, b = (x / AS_TA) % AS_TB, j = (x / (AS_TB * AS_TA)) % AS_TJ, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            double w = 0.0;
             if (aa < bb && bb < v && pij < po) {
                 const int2 ij = op[pij];
                 const long long ia = off + (long long)ij.x * v + aa, jb = off + (long long)ij.y * v + bb, ja = off + (long long)ij.y * v + aa, ib = off + (long long)ij.x * v + bb;
-                acc[pl][j][a][b] += -A.Zsc[ib * ld + pl * (long long)d.n1 + ja] + A.Zsc[jb * ld + pl * (long long)d.n1 + ia];
+                w = -Zsc[ib * ld + pl * n1 + ja] + Zsc[jb * ld + pl * n1 + ia];
             }
+            val[it] = w;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][(x / (AS_TB * AS_TA)) % AS_TJ][x % AS_TA][(x / AS_TA) % AS_TB] += val[it];
         }
         __syncthreads();
         // class "pair (ij) fastest": ladder output and its T1 corrections
-        for (int x = tid; x < 2 * AS_TJ * AS_TA * AS_TB; x += 256) {
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
             const int j = x % AS_TJ, b = (x / AS_TJ) % AS_TB, a = (x / (AS_TJ * AS_TB)) % AS_TA, pl = x / (AS_TB * AS_TA * AS_TJ);
             const int bb = b0 + b, aa = a0 + a, pij = p0 + j;
+            double w = 0.0;
             if (aa < bb && bb < v && pij < po) {
                 const long long c = pl * (long long)po + pij;
-                acc[pl][j][a][b] += A.Yss[s][((long long)(o + aa) * d.n + o + bb) * 2 * po + c]
-                                  - A.Zv[s][((long long)aa * v + bb) * 2 * po + c] + A.Zv[s][((long long)bb * v + aa) * 2 * po + c];
+                w = Yss[((long long)(o + aa) * d.n + o + bb) * 2 * po + c] - Zv[((long long)aa * v + bb) * 2 * po + c] + Zv[((long long)bb * v + aa) * 2 * po + c];
             }
+            val[it] = w;
+        }
+#pragma unroll
+        for (int it = 0; it < AS_NIT; ++it) {
+            const int x = tid + it * 256;
+            acc[x / (AS_TB * AS_TA * AS_TJ)][x % AS_TJ][(x / (AS_TJ * AS_TB)) % AS_TA][(x / AS_TJ) % AS_TB] += val[it];
         }
         __syncthreads();
         // packed output: pair(a,b) = b(b-1)/2 + a, a fastest

@@ -632,7 +632,7 @@ inline void ladder_probe_occupancy(LadderOcc& o, int num_sms)
 // Cluster size and column groups for ncol column tiles.  A CTA holds at most LW_MAXC tiles; the W chunks are rebuilt once per
 // group, so the fewest groups win, then the estimated time  (W1 + cl * ceil(tiles / cl) * W2) / active SMs  per row tile and
 // chunk (W1: building one chunk, W2: applying it to one column tile; the busiest CTA of the cluster sets the pace).
-struct LadderTune { int max_cluster = 16, force_cluster = 0, max_tiles = LW_MAXC, force_split = 0; };
+struct LadderTune { int max_cluster = 16, force_cluster = 0, max_tiles = LW_MAXC, force_split = 0, overlap = 1; };
 inline void ladder_choose_cluster(int ncol, int NQ, const LadderOcc& occ, const LadderTune& tune, int& cl_out, int& ngrp_out)
 {
     const double W1 = 128.0 * 64.0 * NQ, W2 = 64.0 * 128.0 * 128.0;
@@ -750,7 +750,10 @@ inline double ladder_flops(const LadderBatch& b)
     return f;
 }
 
-inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
+// side / ev_fork / ev_join (optional): the second and later wide launches go to `side` so that their CTAs fill the partly
+// empty last wave of the first one (one CTA per SM: launches on one stream would each end in their own tail); `st` waits for them.
+inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms, cudaStream_t side = nullptr,
+                         cudaEvent_t ev_fork = nullptr, cudaEvent_t ev_join = nullptr, int overlap = 1)
 {
     int launches = 0;
     bool red = false;
@@ -760,30 +763,41 @@ inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms)
         ladder_kernel<<<b.nitems, LD_NTH, ladder_smem(), st>>>(pb);
         ++launches;
     }
+    // the wide launches, one per cluster size
+    LadderWide wl[3]; long long wcl[3]; int nwl = 0;
     for (int i = 0; i < b.ncase; ++i) {
         const LadderCase& g = b.c[i];
         red |= g.nsplit > 1;
         if (g.cl <= 0 || g.ntiles <= 0) continue;
         bool first = true;
-        for (int k = 0; k < i; ++k) first &= b.c[k].cl != g.cl;
+        for (int k = 0; k < i; ++k) first &= b.c[k].cl != g.cl || b.c[k].ntiles <= 0;
         if (!first) continue;
-        LadderWide w;
+        LadderWide& w = wl[nwl];
         w.ncase = 0; w.NQ = b.NQ; w.cl = g.cl;
         long long clusters = 0;
         for (int k = i; k < b.ncase; ++k)
             if (b.c[k].cl == g.cl && b.c[k].ntiles > 0) { w.c[w.ncase++] = b.c[k]; clusters += (long long)b.c[k].ntiles * b.c[k].ngrp * b.c[k].nsplit; }
+        wcl[nwl++] = clusters;
+    }
+    bool forked = false;
+    if (nwl > 1 && overlap && side && ev_fork && ev_join) {  // fork BEFORE the first wide launch: `side` must not wait for it
+        cudaEventRecord(ev_fork, st); cudaStreamWaitEvent(side, ev_fork, 0); forked = true;
+    }
+    for (int u = 0; u < nwl; ++u) {
+        const int i = overlap == 2 ? nwl - 1 - u : u;
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(clusters * g.cl));
+        cfg.gridDim = dim3((unsigned)(wcl[i] * wl[i].cl));
         cfg.blockDim = dim3(LW_NTH);
         cfg.dynamicSmemBytes = ladder_wide_smem();
-        cfg.stream = st;
+        cfg.stream = (u > 0 && forked) ? side : st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = (unsigned)g.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        at[0].val.clusterDim.x = (unsigned)wl[i].cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, ladder_wide_kernel, w);
+        cudaLaunchKernelEx(&cfg, ladder_wide_kernel, wl[i]);
         ++launches;
     }
+    if (forked) { cudaEventRecord(ev_join, side); cudaStreamWaitEvent(st, ev_join, 0); }
     if (red) { ladder_reduce_kernel<<<num_sms * 4, 256, 0, st>>>(b); ++launches; }
     return launches;
 }

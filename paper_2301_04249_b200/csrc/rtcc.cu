@@ -5,6 +5,7 @@
 // (tcgemm.cuh) except the particle-particle ladder (ladder.cuh); the rest is elementwise.cuh.
 #include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <string>
 #include <utility>
@@ -33,6 +34,7 @@ struct rtcc_ctx {
     cudaStream_t st = nullptr;
     cudaStream_t S[8]{};                 // S[0] = st (or the capture stream), S[1..3] = helper branches
     cudaStream_t aux[7]{};
+    cudaStream_t lad_side = nullptr; cudaEvent_t lad_ev[2]{};   // second wide ladder launch runs beside the first
     cudaEvent_t evs[16]{};
     int si = 0;
     int sec = 0; unsigned skipmask = 0;   // debug: RTCC_SKIP_MASK skips the GEMMs of pipeline sections (timing experiments only)
@@ -219,8 +221,21 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     // ---- 1. unpack the packed spin blocks into the contraction layouts
     c->sec = 1;
     EW(c, k_unpack_t1, n1, d, t1p, c->t1r);
-    EW(c, k_build_Tsc, (long long)n1 * n1, d, t2p, c->Tsc, c->ring3m ? c->Ts_sc : nullptr);
-    EW(c, k_build_TAB, (long long)d.nA * d.nB, d, t2p, c->TAB, c->ring3m ? c->Ts_AB : nullptr);
+    {   // pair-space matrices T_sc, T_AB (and Re + Im for the three-multiplication products): every packed amplitude read once
+        double* Ts = c->ring3m ? c->Ts_sc : nullptr;
+        const long long nab = (long long)d.oo * ((d.v[0] + UP_T - 1) / UP_T) * ((d.v[1] + UP_T - 1) / UP_T);
+        if (nab > 0) {
+            k_unpack_ab<<<(int)std::min<long long>(nab, (long long)c->num_sms * 16), 256, 0, ST>>>(d, t2p, c->Tsc, c->TAB, Ts, c->ring3m ? c->Ts_AB : nullptr);
+            c->launches++;
+        }
+        for (int s = 0; s < 2; ++s) {
+            const long long nT = (d.v[s] + UP_T - 1) / UP_T, nss = (long long)d.po[s] * (nT * (nT + 1) / 2);
+            if (nss > 0) {
+                k_unpack_ss<<<(int)std::min<long long>(nss, (long long)c->num_sms * 16), 256, 0, ST>>>(d, s, c->opairs[s], t2p, c->Tsc, Ts);
+                c->launches++;
+            }
+        }
+    }
     EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
     for (int s = 0; s < 2; ++s)
         if (d.po[s] > 0)
@@ -576,7 +591,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     BR(3);
     WAITEV(3, 0);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
-    c->launches += ladder_launch(c->lb, ST, c->num_sms);
+    c->launches += ladder_launch(c->lb, ST, c->num_sms, c->lad_side, c->lad_ev[0], c->lad_ev[1], c->opt.lad.overlap);
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], ST));
@@ -1153,7 +1168,7 @@ int residual_pipeline_lean(rtcc_ctx* c, const double* x, double* r)
                (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s]);
         }
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], STL));
-    c->launches += ladder_launch(c->lb, STL, c->num_sms);
+    c->launches += ladder_launch(c->lb, STL, c->num_sms, c->lad_side, c->lad_ev[0], c->lad_ev[1], c->opt.lad.overlap);
     c->flops += ladder_flops(c->lb);
     c->lad_flops = ladder_flops(c->lb);
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[1], STL));
@@ -1451,6 +1466,7 @@ int rtcc_set_default_option(const char* name, int value)
     else if (k == "ladder_split") { if (value < 0 || value > 64) return RTCC_EINVAL; g_opt.lad.force_split = value; }
     else if (k == "max_cluster") { if (value < 1 || value > 16) return RTCC_EINVAL; g_opt.lad.max_cluster = value; }
     else if (k == "ladder_cluster") { if (value < 0 || value > 16) return RTCC_EINVAL; g_opt.lad.force_cluster = value; }
+    else if (k == "ladder_overlap") { if (value < 0 || value > 2) return RTCC_EINVAL; g_opt.lad.overlap = value; }
     else if (k == "ladder_tiles") { if (value < 1 || value > LW_MAXC) return RTCC_EINVAL; g_opt.lad.max_tiles = value; }
     else if (k == "lean") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.lean = value; }
     else if (k == "ring_3m") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.ring3m = value; }
@@ -1468,6 +1484,8 @@ void rtcc_destroy(rtcc_ctx* c)
     if (c->ev[1]) cudaEventDestroy(c->ev[1]);
     if (c->ev_delta) cudaEventDestroy(c->ev_delta);
     for (int i = 0; i < 7; ++i) if (c->aux[i]) cudaStreamDestroy(c->aux[i]);
+    if (c->lad_side) cudaStreamDestroy(c->lad_side);
+    for (int i = 0; i < 2; ++i) if (c->lad_ev[i]) cudaEventDestroy(c->lad_ev[i]);
     for (int i = 0; i < 16; ++i) if (c->evs[i]) cudaEventDestroy(c->evs[i]);
     for (void* p : c->allocs) cudaFree(p);
     if (c->h_scal) cudaFreeHost(c->h_scal);
@@ -1538,8 +1556,10 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             const bool prio = c->opt.prio != 0;
             for (int i = 0; i < 7; ++i)
                 CKC(cudaStreamCreateWithPriority(&c->aux[i], cudaStreamNonBlocking, (prio && i != 2) ? hi : lo));
+            CKC(cudaStreamCreateWithPriority(&c->lad_side, cudaStreamNonBlocking, lo));
         }
         for (int i = 0; i < 16; ++i) CKC(cudaEventCreateWithFlags(&c->evs[i], cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) CKC(cudaEventCreateWithFlags(&c->lad_ev[i], cudaEventDisableTiming));
         for (int i = 0; i < 8; ++i) c->S[i] = c->st;
         c->si = 0;
 #ifdef RTCC_DEBUG_KNOBS
@@ -1624,6 +1644,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
         DA(c->t1r, 2LL * n1, "t1r");
         if (!c->lean) {
             DA(c->Tsc, 2LL * n1 * n1, "Tsc");
+            CKC(cudaMemsetAsync(c->Tsc, 0, (size_t)(2LL * n1 * n1 > 0 ? 2LL * n1 * n1 : 1) * 8, c->st));   // i == m / a == e places stay zero
             DA(c->Wsc, 2LL * n1 * n1, "Wsc");
             DA(c->Zsc, 2LL * n1 * n1, "Zsc");
             DA(c->TAB, 2LL * d.nA * d.nB, "TAB");
@@ -1633,6 +1654,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             DA(c->ZBA, 2LL * d.nB * d.nA, "ZBA");
             if (c->ring3m) {
                 DA(c->Ts_sc, (long long)n1 * n1, nullptr);
+                CKC(cudaMemsetAsync(c->Ts_sc, 0, (size_t)((long long)n1 * n1 > 0 ? (long long)n1 * n1 : 1) * 8, c->st));
                 DA(c->Wd_sc, (long long)n1 * n1, nullptr);
                 DA(c->Ts_AB, (long long)d.nA * d.nB, nullptr);
                 DA(c->Wd_BB, (long long)d.nB * d.nB, nullptr);
