@@ -70,6 +70,9 @@ void rtcc_destroy(rtcc_ctx* ctx);
  *   "max_cluster" (16)      largest thread-block cluster the wide ladder kernel may use (1..16)
  *   "ladder_cluster" (0)    0: automatic, k >= 1: force clusters of k CTAs in the wide ladder kernel
  *   "ladder_tiles" (5)      column tiles one CTA of the wide ladder kernel may hold (1..5; 4 of them parked in tensor memory)
+ *   "ladder_overlap" (1)    wide ladder launches of different cluster sizes: 0 one after the other on one stream; 1 side by side,
+ *                           the launch with the longest CTAs first and the others on a helper stream, so that their CTAs fill
+ *                           its last, partly empty wave; 2 side by side, shortest first (for comparison)
  *   "lean" (-1)             -1: low-memory layout only when the standard one does not fit, 0: never, 1: always
  *   "ring_3m" (-1)          complex x complex ring products T.W by three real multiplications instead of four (same result up to
  *                           rounding): -1 automatic (pair space >= 1536 and the two extra matrices fit), 0 never, 1 always

@@ -783,8 +783,26 @@ inline int ladder_launch(const LadderBatch& b, cudaStream_t st, int num_sms, cud
     if (nwl > 1 && overlap && side && ev_fork && ev_join) {  // fork BEFORE the first wide launch: `side` must not wait for it
         cudaEventRecord(ev_fork, st); cudaStreamWaitEvent(side, ev_fork, 0); forked = true;
     }
+    // side by side: longest CTAs first (their tail is filled by the shorter CTAs of the later launches)
+    int ord[3] = {0, 1, 2};
+    if (overlap) {
+        double cost[3];
+        for (int i = 0; i < nwl; ++i) {
+            int per = 0;
+            for (int k = 0; k < wl[i].ncase; ++k) {
+                const LadderCase& g = wl[i].c[k];
+                const int ng = (g.ncol + g.ngrp - 1) / g.ngrp, p = (ng + g.cl - 1) / g.cl;
+                if (p > per) per = p;
+            }
+            cost[i] = 128.0 * 64.0 * b.NQ / wl[i].cl + per * 64.0 * 128.0 * 128.0;
+            if (overlap == 2) cost[i] = -cost[i];
+        }
+        for (int i = 0; i < nwl; ++i)
+            for (int k = i + 1; k < nwl; ++k)
+                if (cost[ord[k]] > cost[ord[i]]) { const int t = ord[i]; ord[i] = ord[k]; ord[k] = t; }
+    }
     for (int u = 0; u < nwl; ++u) {
-        const int i = overlap == 2 ? nwl - 1 - u : u;
+        const int i = ord[u];
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)(wcl[i] * wl[i].cl));
         cfg.blockDim = dim3(LW_NTH);
