@@ -70,6 +70,8 @@ void rtcc_destroy(rtcc_ctx* ctx);
  *   "max_cluster" (16)      largest thread-block cluster the wide ladder kernel may use (1..16)
  *   "ladder_cluster" (0)    0: automatic, k >= 1: force clusters of k CTAs in the wide ladder kernel
  *   "ladder_tiles" (5)      column tiles one CTA of the wide ladder kernel may hold (1..5; 4 of them parked in tensor memory)
+ *   "ladder_antisym" (1)    wide ladder kernel, same-spin cases: visit only (e,f) chunks that hold an e < f, two W products per
+ *                           chunk combined to (pe|qf) - (pf|qe), one application (0: every (e,f) chunk, one product each)
  *   "ladder_overlap" (1)    wide ladder launches of different cluster sizes: 0 one after the other on one stream; 1 side by side,
  *                           the launch with the longest CTAs first and the others on a helper stream, so that their CTAs fill
  *                           its last, partly empty wave; 2 side by side, shortest first (for comparison)

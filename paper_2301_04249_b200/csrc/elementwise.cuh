@@ -220,7 +220,7 @@ __global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double
 
 // X_ss[(e,f)][pl][(i<j)] = t_{ij}^{ef};  tau = X + t1[i,e] t1[j,f] - t1[i,f] t1[j,e]
 __global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const double* __restrict__ t1r,
-                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau)
+                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau, int anti)
 {
     const int v = d.v[s], po = d.po[s];
     const long long tot = (long long)v * v * po;
@@ -236,8 +236,10 @@ __global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const
         double ti = t1r[ie] * t1r[d.n1 + jf] + t1r[d.n1 + ie] * t1r[jf] - (t1r[iff] * t1r[d.n1 + je] + t1r[d.n1 + iff] * t1r[je]);
         X[row * 2 * po + col] = z.re;
         X[row * 2 * po + po + col] = z.im;
-        Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
-        Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;
+        if (!anti || e < f) {                 // antisymmetrised ladder: rows e >= f stay zero (cleared at creation)
+            Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
+            Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;
+        }
         tau[row * 2 * po + col] = z.re + tr;
         tau[row * 2 * po + po + col] = z.im + ti;
     }
@@ -598,7 +600,7 @@ __global__ void k_build_Xt_ab(Dims d, const double* __restrict__ t2p, double* __
         Xt[xt_index(e, F, d.oo + col, nFt, ncol, nt2)] = t2p[2 * k + 1];
     }
 }
-__global__ void k_build_Xt_ss(Dims d, int s, const double* __restrict__ t2p, const int2* __restrict__ opairs, double* __restrict__ Xt, int nFt, int ncol, int nt2)
+__global__ void k_build_Xt_ss(Dims d, int s, const double* __restrict__ t2p, const int2* __restrict__ opairs, double* __restrict__ Xt, int nFt, int ncol, int nt2, int anti)
 {
     const int v = d.v[s], po = d.po[s];
     const long long tot = (long long)v * v * po;
@@ -606,6 +608,7 @@ __global__ void k_build_Xt_ss(Dims d, int s, const double* __restrict__ t2p, con
         const long long row = x / po; const int col = (int)(x - row * po);
         const int e = (int)(row / v), f = (int)(row - (long long)e * v);
         const int2 ij = opairs[col];
+        if (anti && e >= f) continue;         // antisymmetrised ladder: those rows stay zero
         c128 z = ss_amp(t2p, d.off_t2[s], d.pv[s], ij.x, ij.y, e, f);
         Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
         Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;

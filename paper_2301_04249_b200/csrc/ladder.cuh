@@ -42,7 +42,18 @@ struct LadderCase {
     int cl;                               // 0: batched narrow kernel (one column tile); >= 1: wide kernel, CTAs per cluster
     int ngrp;                             // wide kernel: column-tile groups (each group rebuilds the W chunks)
     int item0;                            // first work item of this case
+    int same;                             // p and q (e and f) are of the same spin: X is antisymmetric in (e,f), Y in (p,q)
+    int anti;                             // wide kernel, same spin: chunks with e < f only, W antisymmetrised (see ladder_wide_kernel)
 };
+// (e,f) chunks of a case: all nEt x nFt, or -- antisymmetrised -- those that hold an e < f: ft >= 2 et (16 e x 8 f per chunk)
+__host__ __device__ inline int ladder_nchunk(int vA, int vB, int anti)
+{
+    const int nEt = (vA + 15) / 16, nFt = (vB + 7) / 8;
+    if (!anti) return nEt * nFt;
+    int n = 0;
+    for (int et = 0; et < nEt && 2 * et < nFt; ++et) n += nFt - 2 * et;
+    return n;
+}
 struct LadderBatch {
     LadderCase c[3];
     int ncase, NQ, nitems;                // NQ: padded to a multiple of 16
@@ -343,6 +354,23 @@ __device__ __forceinline__ void tmem_zero64(unsigned taddr)
     tmem_wait_st();
 }
 
+// park this thread's 32 accumulators at taddr (64 columns), same element order as tmem_exchange
+__device__ __forceinline__ void tmem_put(unsigned taddr, const double (&acc)[4][4][2])
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+            tmem_st8(taddr + 16 * i + 8 * h, acc[i][2 * h][0], acc[i][2 * h][1], acc[i][2 * h + 1][0], acc[i][2 * h + 1][1]);
+    tmem_wait_st();
+}
+
+// Antisymmetrised same-spin form (LadderCase::anti).  X^{ef} = -X^{fe}, so
+//   Y^{pq} = sum_{e<f} [ (pe|qf) - (pf|qe) ] X^{ef}:
+// only chunks that hold an e < f are visited (rows e >= f of the tile-major X are zero), each with TWO W products -- first
+// (pe|qf) from the (p0, et) x (q0, ft) operand tiles, parked in the free tensor-memory slot, then (qe|pf) = (pf|qe) from the
+// (q0, et) x (p0, ft) tiles -- combined in the shared-memory slot, and ONE application: the same W-build flops as the plain form
+// (which visits every (e,f)), about half the apply flops.  A CTA then holds at most 4 column tiles (one slot is the parking place).
 __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide b)
 {
     constexpr int NT2 = 128, LDX2 = NT2 + 4, T2 = LD_K2 / LD_BK;
@@ -374,10 +402,12 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
     const int ct0 = gt0 + (int)((long long)rank * (gt1 - gt0) / cl), ct1 = gt0 + (int)((long long)(rank + 1) * (gt1 - gt0) / cl);
     const int Ct = ct1 - ct0;                                                 // 0 .. LW_MAXC
     const int nEt = (g.vA + LD_PE - 1) / LD_PE, nFt = (g.vB + LD_PF - 1) / LD_PF;
-    const int nchunk = nEt * nFt;
+    const int anti = g.anti;
+    const int nchunk = ladder_nchunk(g.vA, g.vB, anti);
     const int ch0 = (int)((long long)split * nchunk / g.nsplit), ch1 = (int)((long long)(split + 1) * nchunk / g.nsplit);
     const int G = ch1 - ch0;
     const int T1 = NQ / LD_BK;
+    const int TB = anti ? 2 * T1 : T1;                                       // k-tiles of one W build
 
     if (tid == 0) {
         for (int s = 0; s < LW_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
@@ -407,32 +437,42 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
             const double* LAp = g.LA + (long long)(p0 / LD_PP) * nEt * T1 * BLKA;
             const double* LBp = g.LB + (long long)(q0 / LD_PQ) * nFt * T1 * BLKB;
             int stage = 0; unsigned par = 1;
+            // second product of the antisymmetrised form: rows (q, e), columns (p, f)
+            const double* LAq = g.LA + (long long)(q0 / LD_PP) * nEt * T1 * BLKA;
+            const double* LBq = g.LB + (long long)(p0 / LD_PQ) * nFt * T1 * BLKB;
+            auto chunk_ef = [&](int ch, int& et, int& ft) {
+                if (!anti) { et = ch / nFt; ft = ch % nFt; return; }
+                et = 0;
+                while (ch >= nFt - 2 * et) { ch -= nFt - 2 * et; ++et; }
+                ft = 2 * et + ch;
+            };
             auto issue_L = [&](int ch, int k0, int k1) {
-                const int et = ch / nFt, ft = ch % nFt;
-                const double* curA = LAp + ((long long)et * T1 + k0) * BLKA;
-                const double* curB = LBp + ((long long)ft * T1 + k0) * BLKB;
+                int et, ft;
+                chunk_ef(ch, et, ft);
                 for (int t = k0; t < k1; ++t) {
+                    const int tt = t < T1 ? t : t - T1;
+                    const double* curA = (t < T1 ? LAp : LAq) + ((long long)et * T1 + tt) * BLKA;
+                    const double* curB = (t < T1 ? LBp : LBq) + ((long long)ft * T1 + tt) * BLKB;
                     mbar_wait(&empty[stage], par);
                     double* sb = stg + stage * LD_STAGE;
                     mbar_expect_tx(&full[stage], (BLKA + BLKB) * 8);
                     bulk_g2s(sb, curA, BLKA * 8, &full[stage]);
                     bulk_g2s(sb + BLKA, curB, BLKB * 8, &full[stage]);
-                    curA += BLKA; curB += BLKB;
                     if (++stage == LW_ST) { stage = 0; par ^= 1; }
                 }
             };
             int gb = rank, kdone = 0;
             for (int s = -2; s < G; ++s) {
                 if (s >= -1 && s + 1 < G && (s + 1) % cl == rank) { gb = s + 1 + cl; kdone = 0; }
-                if (gb < G && kdone < T1) {
+                if (gb < G && kdone < TB) {
                     const int rem = gb - 1 - s;
-                    const int nk = (T1 - kdone + rem - 1) / rem;
+                    const int nk = (TB - kdone + rem - 1) / rem;
                     issue_L(ch0 + gb, kdone, kdone + nk);
                     kdone += nk;
                 }
                 if (s >= 0 && Ct > 0) {
-                    const int ch = ch0 + s;
-                    const int et = ch / nFt, ft = ch % nFt;
+                    int et, ft;
+                    chunk_ef(ch0 + s, et, ft);
                     const double* Xc = g.X + ((long long)(et * nFt + ft) * g.ncol) * T2 * BLKX;
                     for (int u = 0; u < Ct; ++u) {
                         const int tile = (s & 1) ? Ct - 1 - u : u;
@@ -463,6 +503,7 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
         // this warp's tensor-memory region: lanes 32 (warp % 4) .., columns 256 (warp / 4) + 64 slot
         const unsigned tm0 = tmem_base + ((unsigned)((warp & 3) * 32) << 16) + (unsigned)((warp >> 2) * 256);
         for (int s = 0; s + 1 < Ct; ++s) tmem_zero64(tm0 + 64 * s);      // parked tiles start at zero
+        const unsigned tm_stash = tm0 + 64 * (LW_MAXC - 2);                  // antisymmetrised form: parking place of the first W product
 
         int stage = 0; unsigned par = 0;
         unsigned cpar = 0u;                                                   // bit sl: parity of credit[sl]
@@ -471,6 +512,44 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
             const int sl = gc & 1;
             if (gc >= 2) { mbar_wait_cluster(&credit[sl], (cpar >> sl) & 1u); cpar ^= 1u << sl; }     // every warp of the cluster is done with chunk gc-2
             double* Ws = Wsl + sl * LW_WSLOT;
+            if (anti) {
+                // first product back from tensor memory into its places, then the second one subtracted at the places of the
+                // transposed (p,q) -- other threads' elements, hence the barrier in between
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int m = w1m + 8 * i + lr;
+                    const int p = m / LD_PE, e = m % LD_PE;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        unsigned in[8];
+                        tmem_ld8(tm_stash + 16 * i + 8 * h, in);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int jj = 0; jj < 2; ++jj) {
+                            const int n = w1n + 8 * (2 * h + jj) + 2 * lc;
+                            const int q = n / LD_PF, f = n % LD_PF;
+                            *reinterpret_cast<double2*>(&Ws[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]) =
+                                make_double2(__hiloint2double((int)in[4 * jj + 1], (int)in[4 * jj]), __hiloint2double((int)in[4 * jj + 3], (int)in[4 * jj + 2]));
+                        }
+                    }
+                }
+                bar_consumers();
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int m = w1m + 8 * i + lr;
+                    const int q = m / LD_PE, e = m % LD_PE;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int n = w1n + 8 * j + 2 * lc;
+                        const int p = n / LD_PF, f = n % LD_PF;
+                        double2* w = reinterpret_cast<double2*>(&Ws[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]);
+                        double2 v = *w;
+                        v.x -= acc1[i][j][0]; v.y -= acc1[i][j][1];
+                        *w = v;
+                        acc1[i][j][0] = acc1[i][j][1] = 0.0;
+                    }
+                }
+            } else {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int m = w1m + 8 * i + lr;
@@ -482,6 +561,7 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
                     *reinterpret_cast<double2*>(&Ws[(p * LD_PQ + q) * LD_LDW + e * LD_PF + f]) = make_double2(acc1[i][j][0], acc1[i][j][1]);
                     acc1[i][j][0] = acc1[i][j][1] = 0.0;
                 }
+            }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes -> visible to the bulk copies
             bar_consumers();
@@ -498,11 +578,19 @@ __global__ void __launch_bounds__(LW_NTH, 1) ladder_wide_kernel(const LadderWide
         int gb = rank, kdone = 0;
         for (int s = -2; s < G; ++s) {
             if (s >= -1 && s + 1 < G && (s + 1) % cl == rank) { publish(s + 1); gb = s + 1 + cl; kdone = 0; }
-            if (gb < G && kdone < T1) {
+            if (gb < G && kdone < TB) {
                 const int rem = gb - 1 - s;
-                const int nk = (T1 - kdone + rem - 1) / rem;
+                const int nk = (TB - kdone + rem - 1) / rem;
+                const int kfirst = kdone;
                 kdone += nk;
                 for (int t = 0; t < nk; ++t) {
+                    if (anti && kfirst + t == T1) {                           // first product complete: park it, start the second
+                        tmem_put(tm_stash, acc1);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
+                    }
                     mbar_wait(&full[stage], par);
                     const double* sb = stg + stage * LD_STAGE;
                     const double* as = sb + lc * LD_LDA1 + w1m + lr;
@@ -632,10 +720,12 @@ inline void ladder_probe_occupancy(LadderOcc& o, int num_sms)
 // Cluster size and column groups for ncol column tiles.  A CTA holds at most LW_MAXC tiles; the W chunks are rebuilt once per
 // group, so the fewest groups win, then the estimated time  (W1 + cl * ceil(tiles / cl) * W2) / active SMs  per row tile and
 // chunk (W1: building one chunk, W2: applying it to one column tile; the busiest CTA of the cluster sets the pace).
-struct LadderTune { int max_cluster = 16, force_cluster = 0, max_tiles = LW_MAXC, force_split = 0, overlap = 1; };
-inline void ladder_choose_cluster(int ncol, int NQ, const LadderOcc& occ, const LadderTune& tune, int& cl_out, int& ngrp_out)
+struct LadderTune { int max_cluster = 16, force_cluster = 0, max_tiles = LW_MAXC, force_split = 0, overlap = 1, anti = 1; };
+inline void ladder_choose_cluster(int ncol, int NQ, const LadderOcc& occ, const LadderTune& tune_in, int anti, int& cl_out, int& ngrp_out)
 {
-    const double W1 = 128.0 * 64.0 * NQ, W2 = 64.0 * 128.0 * 128.0;
+    LadderTune tune = tune_in;
+    if (anti && tune.max_tiles > LW_MAXC - 1) tune.max_tiles = LW_MAXC - 1;     // one tensor-memory slot parks the first W product
+    const double W1 = 128.0 * 64.0 * NQ * (anti ? 2 : 1), W2 = 64.0 * 128.0 * 128.0;
     int maxc = 16, minc = 1;
     if (tune.max_cluster >= 1 && tune.max_cluster < maxc) maxc = tune.max_cluster;
     if (tune.force_cluster >= 1 && tune.force_cluster <= 16 && occ.act[tune.force_cluster] > 0) minc = maxc = tune.force_cluster;
@@ -664,17 +754,21 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const Ladder
         g.nt2 = g.N2 <= 64 ? 64 : 128;
         g.ncol = (g.N2 + g.nt2 - 1) / g.nt2;
         g.cl = 0; g.ngrp = 1;                 // cl = 0: batched narrow kernel
-        if (g.ncol > 1) ladder_choose_cluster(g.ncol, b.NQ, occ, tune, g.cl, g.ngrp);
+        g.anti = (g.same && g.ncol > 1 && tune.anti) ? 1 : 0;
+        if (g.ncol > 1) ladder_choose_cluster(g.ncol, b.NQ, occ, tune, g.anti, g.cl, g.ngrp);
         else rows += g.ntiles;
     }
     // One launch for all wide cases when a common cluster size costs no case more than 3 % (modelled): separate launches
     // each end in a partly filled last wave.
     {
-        const double W1 = 128.0 * 64.0 * b.NQ, W2 = 64.0 * 128.0 * 128.0;
+        const double W2 = 64.0 * 128.0 * 128.0;
         auto cost = [&](const LadderCase& g, int cl) {
             if (cl < 1 || cl > 16 || occ.act[cl] <= 0) return 1e300;
+            const double W1 = 128.0 * 64.0 * b.NQ * (g.anti ? 2 : 1);
             const int ng = (g.ncol + g.ngrp - 1) / g.ngrp, per = (ng + cl - 1) / cl;
-            if (per > (tune.max_tiles >= 1 && tune.max_tiles < LW_MAXC ? tune.max_tiles : LW_MAXC)) return 1e300;
+            int maxt = tune.max_tiles >= 1 && tune.max_tiles < LW_MAXC ? tune.max_tiles : LW_MAXC;
+            if (g.anti && maxt > LW_MAXC - 1) maxt = LW_MAXC - 1;
+            if (per > maxt) return 1e300;
             return (W1 + (double)cl * per * W2) / occ.act[cl];
         };
         int common = 0;
@@ -703,7 +797,7 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const Ladder
     int item = 0;
     for (int i = 0; i < b.ncase; ++i) {
         LadderCase& g = b.c[i];
-        const int nchunk = ((g.vA + LD_PE - 1) / LD_PE) * ((g.vB + LD_PF - 1) / LD_PF);
+        const int nchunk = ladder_nchunk(g.vA, g.vB, g.anti);
         g.item0 = 0;
         if (g.cl == 0) {
             g.nsplit = best < nchunk ? best : (nchunk > 0 ? nchunk : 1);
@@ -730,7 +824,7 @@ inline void ladder_plan(LadderBatch& b, int num_sms, int max_split, const Ladder
         for (int k = i; k < b.ncase; ++k) {
             LadderCase& h = b.c[k];
             if (h.cl != g.cl) continue;
-            const int nchunk = ((h.vA + LD_PE - 1) / LD_PE) * ((h.vB + LD_PF - 1) / LD_PF);
+            const int nchunk = ladder_nchunk(h.vA, h.vB, h.anti);
             h.nsplit = S < nchunk ? S : (nchunk > 0 ? nchunk : 1);
             h.item0 = it;
             it += h.ntiles * h.ngrp * h.nsplit;
@@ -745,7 +839,8 @@ inline double ladder_flops(const LadderBatch& b)
     for (int i = 0; i < b.ncase; ++i) {
         const LadderCase& g = b.c[i];
         double rows = 64.0 * g.ntiles, ef = (double)g.vA * g.vB;
-        f += 2.0 * rows * ef * ((double)b.NQ * g.ngrp + (double)g.ncol * g.nt2);
+        if (g.anti) ef *= (double)ladder_nchunk(g.vA, g.vB, 1) / ladder_nchunk(g.vA, g.vB, 0);      // chunks visited; two W products each
+        f += 2.0 * rows * ef * ((double)b.NQ * g.ngrp * (g.anti ? 2 : 1) + (double)g.ncol * g.nt2);
     }
     return f;
 }

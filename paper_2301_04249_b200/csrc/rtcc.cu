@@ -53,6 +53,7 @@ struct rtcc_ctx {
     double *Xab = nullptr, *tauab = nullptr, *Yab = nullptr, *Wooab = nullptr;
     double *LtA[2]{}, *LtB[2]{}, *Xt_ab = nullptr, *Xt_ss[2]{};   // tile-major ladder operands
     int nt2_ab = 128, nt2_ss[2]{128, 128};
+    int anti_ss[2]{0, 0};                 // same-spin ladder in the antisymmetrised form: rows e >= f of the tile-major X stay zero
     double *Xss[2]{}, *tauss[2]{}, *Yss[2]{}, *W4[2]{}, *Wp[2]{}, *Yoop[2]{}, *Zv[2]{};
     int2 *opairs[2]{}, *vpairs[2]{}, *tiles_ab = nullptr, *tiles_ss[2]{};
     int ntiles_ab = 0, ntiles_ss[2]{};
@@ -239,7 +240,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
     for (int s = 0; s < 2; ++s)
         if (d.po[s] > 0)
-            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->Xt_ss[s], (d.v[s] + 7) / 8, (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->tauss[s]);
+            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->Xt_ss[s], (d.v[s] + 7) / 8, (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->tauss[s], c->anti_ss[s]);
 
     if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
 
@@ -1165,7 +1166,7 @@ int residual_pipeline_lean(rtcc_ctx* c, const double* x, double* r)
         if (d.po[s] > 0) {
             CK(cudaMemsetAsync(c->Xt_ss[s], 0, (size_t)c->xt_ss_cnt[s] * 8, STL));
             EW(c, k_build_Xt_ss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->opairs[s], c->Xt_ss[s], (d.v[s] + 7) / 8,
-               (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s]);
+               (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->anti_ss[s]);
         }
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], STL));
     c->launches += ladder_launch(c->lb, STL, c->num_sms, c->lad_side, c->lad_ev[0], c->lad_ev[1], c->opt.lad.overlap);
@@ -1466,6 +1467,7 @@ int rtcc_set_default_option(const char* name, int value)
     else if (k == "ladder_split") { if (value < 0 || value > 64) return RTCC_EINVAL; g_opt.lad.force_split = value; }
     else if (k == "max_cluster") { if (value < 1 || value > 16) return RTCC_EINVAL; g_opt.lad.max_cluster = value; }
     else if (k == "ladder_cluster") { if (value < 0 || value > 16) return RTCC_EINVAL; g_opt.lad.force_cluster = value; }
+    else if (k == "ladder_antisym") g_opt.lad.anti = value != 0;
     else if (k == "ladder_overlap") { if (value < 0 || value > 2) return RTCC_EINVAL; g_opt.lad.overlap = value; }
     else if (k == "ladder_tiles") { if (value < 1 || value > LW_MAXC) return RTCC_EINVAL; g_opt.lad.max_tiles = value; }
     else if (k == "lean") { if (value < -1 || value > 1) return RTCC_EINVAL; g_opt.lean = value; }
@@ -1749,12 +1751,16 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 g.nA = g.nB = n; g.vA = d.v[sa]; g.vB = d.v[sb];
                 g.X = Xt; g.N2 = 2 * cols; g.Y = Y; g.ldY = 2LL * cols; g.Ypart = nullptr;
                 g.tiles = tiles; g.ntiles = ntiles;
+                g.same = sa == sb; g.anti = 0;
             };
             add(0, 1, c->Xt_ab, d.oo, c->Yab, c->tiles_ab, c->ntiles_ab);
             add(0, 0, c->Xt_ss[0], d.po[0], c->Yss[0], c->tiles_ss[0], c->ntiles_ss[0]);
             add(1, 1, c->Xt_ss[1], d.po[1], c->Yss[1], c->tiles_ss[1], c->ntiles_ss[1]);
             ladder_probe_occupancy(c->locc, c->num_sms);
             ladder_plan(B, c->num_sms, 8, c->locc, c->opt.lad);
+            for (int i = 0; i < B.ncase; ++i)
+                for (int s = 0; s < 2; ++s)
+                    if (B.c[i].same && B.c[i].X == c->Xt_ss[s]) c->anti_ss[s] = B.c[i].anti;
             for (int i = 0; i < B.ncase; ++i)
                 if (B.c[i].nsplit > 1) {
                     const long long cnt = (long long)B.c[i].nsplit * nn * B.c[i].ldY;

@@ -73,6 +73,7 @@ def test_residual_general_fock_complex_amplitudes(rtcc, shape):
 @pytest.mark.parametrize("opts", [
     {"ladder_cluster": 2}, {"ladder_cluster": 3}, {"ladder_cluster": 5}, {"ladder_cluster": 4, "ladder_split": 3},
     {"ladder_tiles": 1}, {"ladder_tiles": 2, "ladder_cluster": 2}, {"ladder_tiles": 1, "max_cluster": 2}, {"ladder_split": 2},
+    {"ladder_antisym": 0}, {"ladder_antisym": 0, "ladder_cluster": 3}, {"ladder_overlap": 0}, {"ladder_overlap": 2, "ladder_split": 2},
 ])
 def test_wide_ladder_cluster_shapes(rtcc, opts):
     """The wide ladder kernel's code paths that the automatic plan picks only at larger sizes, forced on a size the full oracle
@@ -116,6 +117,36 @@ def test_wide_ladder_cluster_shapes(rtcc, opts):
 
 
 _WIDE_REF = {}
+
+
+@pytest.mark.parametrize("opts", [{}, {"ladder_antisym": 0}, {"ladder_cluster": 2, "ladder_split": 3}])
+def test_antisymmetrised_same_spin_ladder(rtcc, opts):
+    """Same-spin cases of the wide ladder kernel: only (e,f) chunks with an e < f, two W products per chunk combined to
+    (pe|qf) - (pf|qe) through tensor memory and the shared-memory slot (default), against the plain form and the full oracle, on a
+    shape with 2 x 3 / 2 x 4 chunks (5 / 6 visited), two column tiles per same-spin case, ragged last e and f tiles; also sliced in clusters of 2."""
+    oa, ob, va, vb, K = 13, 12, 24, 25, 19
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=77)
+    d = orc.Dims(oa, ob, va, vb, K)
+    rng = np.random.default_rng(13)
+    t1 = 0.1 * (rng.standard_normal(d.n_t1) + 1j * rng.standard_normal(d.n_t1))
+    t2 = 0.1 * (rng.standard_normal(d.n_t2) + 1j * rng.standard_normal(d.n_t2))
+    if "anti" not in _WIDE_REF:
+        _WIDE_REF["anti"] = orc.Problem(oa, ob, va, vb, K, L, fock).residual(t1, t2)
+    r1o, r2o, Eo = _WIDE_REF["anti"]
+    try:
+        for k, v in opts.items():
+            rtcc.set_default_option(k, v)
+        ctx = rtcc.Rtcc(oa, ob, va, vb, K, L, fock)
+        plan = ctx.ladder_plan()
+        r1, r2 = ctx.residual(t1, t2)
+        ra, rb = ctx.residual(t1, t2)
+        ctx.close()
+    finally:
+        rtcc.set_default_option("reset")
+    scale = max(np.abs(r1o).max(), np.abs(r2o).max())
+    assert np.abs(r2 - r2o).max() <= RTOL * scale and np.abs(r1 - r1o).max() <= RTOL * scale
+    assert np.array_equal(r2, rb) and np.array_equal(r1, ra)
+    assert [p["col_tiles"] for p in plan] == [3, 2, 2] and all(p["cluster"] >= 1 for p in plan)
 
 
 @pytest.mark.parametrize("shape", [(3, 4, 13, 12, 48), (2, 0, 3, 5, 4), (0, 2, 5, 3, 4), (1, 2, 2, 1, 3), (9, 8, 10, 11, 20), (5, 4, 18, 19, 37)])
