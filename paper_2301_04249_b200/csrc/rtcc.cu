@@ -2117,6 +2117,10 @@ int rtcc_step(rtcc_ctx* c, double dt)
     c->E[0] = E_new[0]; c->E[1] = E_new[1];
     c->time += dt;
     c->last_micro = k;
+    if (c->timing) {                      // ladder time of the step's last residual evaluation (the stream is idle: read_scal waited)
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) == cudaSuccess) c->lad_ms = ms; else cudaGetLastError();
+    }
     return RTCC_OK;
 }
 
