@@ -591,6 +591,10 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
     c->sec = 11;
     BR(3);
     WAITEV(3, 0);
+    // same-spin ladder outputs: only row tiles with p-tile <= q-tile are written by the kernel, while the o^4 corrections below
+    // accumulate into every (a,b) row -- clear the buffers so that the rows nobody reads do not grow from evaluation to evaluation
+    for (int s = 0; s < 2; ++s)
+        if (d.po[s] > 0) CK(cudaMemsetAsync(c->Yss[s], 0, (size_t)(nn * 2 * d.po[s]) * 8, ST));
     if (c->timing && !c->capturing) CK(cudaEventRecord(c->ev[0], ST));
     c->launches += ladder_launch(c->lb, ST, c->num_sms, c->lad_side, c->lad_ev[0], c->lad_ev[1], c->opt.lad.overlap);
     c->flops += ladder_flops(c->lb);

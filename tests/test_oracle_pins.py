@@ -485,3 +485,50 @@ def test_spectral_function_closed_forms():
     ref = sum(np.exp(-b) * b ** k / factorial(k) * lor(om - e0 - k * W) for k in range(25))
     assert np.abs(A2 - ref).max() < 2e-4
     assert abs(np.trapezoid(A2, om) - np.trapezoid(ref, om)) < 1e-3
+
+
+# ------------------------------------------------------------------ fixed_micro and set_state of the propagator
+def test_fixed_micro_is_k_sweeps_of_a_contraction_towards_the_implicit_solution():
+    """Eq. 9 is implicit in T(tau+dt); PAPER.md:103 solves it by fixed-point sweeps.  With fixed_micro = k the oracle
+    must do exactly k sweeps: the distance to the converged step (pinned by the exact two-electron dynamics above) then shrinks
+    geometrically in k, by about the same factor per sweep, in both iteration modes; k sweeps of mode 0 started from t and one more
+    differ by exactly one application of the map (checked through the residual the oracle reports)."""
+    oa, ob, va, vb, K = 2, 1, 2, 3, 4
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=5, sigma=0.25, offdiag=0.0)
+    prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+    dt = 0.2
+    for mode in (0, 1):
+        ref = orc.Propagator(prob, mode=mode, tol=1e-15, max_micro=500)
+        ref.step(dt)
+        errs = []
+        for k in range(1, 8):
+            p = orc.Propagator(prob, mode=mode, fixed_micro=k)
+            assert p.step(dt) == k and p.last_micro == k
+            errs.append(max(np.abs(p.t1 - ref.t1).max(), np.abs(p.t2 - ref.t2).max()))
+            if mode == 0 and k >= 2:
+                # the k-th iterate is B + (i dt/2) R(iterate k-1): R(t(k-1)) is what the (k-1)-sweep propagator reports
+                h = 0.5j * dt
+                assert np.allclose(p.t2, h * prob.residual(np.zeros_like(p.t1), np.zeros_like(p.t2))[1] + h * prev.r2, rtol=0, atol=1e-15)
+            prev = p
+        ratios = [errs[i + 1] / errs[i] for i in range(len(errs) - 1)]
+        assert errs[0] > 1e-6 and all(r < 0.8 for r in ratios), (mode, errs)
+        assert max(ratios[1:]) < 4.0 * min(ratios[1:]), (mode, ratios)
+        assert errs[-1] < errs[0] * max(ratios) ** 5 * 1.01
+
+
+def test_set_state_continues_like_the_uninterrupted_run():
+    """Propagator.set_state (the oracle side of the restart tests): a second propagator started from the amplitudes, time and
+    cumulant of the first continues to the same amplitudes and cumulant as the uninterrupted run, and its E at the restart point is
+    the energy functional of those amplitudes."""
+    oa, ob, va, vb, K = 2, 2, 2, 2, 3
+    L, fock = rand_problem(oa, ob, va, vb, K, seed=8, sigma=0.2)
+    prob = orc.Problem(oa, ob, va, vb, K, L, fock)
+    a = orc.Propagator(prob, mode=0, tol=1e-13, max_micro=300)
+    for _ in range(3):
+        a.step(0.05)
+    b = orc.Propagator(prob, mode=0, tol=1e-13, max_micro=300)
+    b.set_state(a.t1, a.t2, a.time, a.C)
+    assert b.E == prob.residual(a.t1, a.t2)[2] and b.time == a.time and b.C == a.C
+    for _ in range(3):
+        a.step(0.05); b.step(0.05)
+    assert np.array_equal(a.t1, b.t1) and np.array_equal(a.t2, b.t2) and a.C == b.C and abs(a.time - 0.3) < 1e-15
