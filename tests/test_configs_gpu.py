@@ -107,6 +107,10 @@ def run_config(rtcc, name, amp_std, n_random, n_r1, max_samples=None, host=False
         r1, r2 = r1d.cpu().numpy(), r2d.cpu().numpy()
     t_gpu = time.time() - t0
     E = ctx.residual_energy()
+    # the closed-form memory budget (rtcc_problem_sizes) against what the context really holds
+    ps = rtcc.problem_sizes(oa, ob, va, vb, K)
+    want = ps["bytes_lean"] if name == "largest" else ps["bytes_standard"]
+    assert abs(ctx.workspace_bytes - want) <= 0.01 * want, (ctx.workspace_bytes, ps)
     assert np.isfinite(r1.view(float)).all() and np.isfinite(r2.view(float)).all()
     scale = max(np.abs(r1).max(), np.abs(r2).max())
     t0 = time.time()
