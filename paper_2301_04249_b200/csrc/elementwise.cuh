@@ -197,51 +197,99 @@ __global__ void __launch_bounds__(256) k_unpack_ss(Dims d, int s, const int2* __
     }
 }
 
+// Ladder operands by tiled transposition (same scheme as k_unpack_*): the packed blocks are [(occupied pair)][(virtual pair)]
+// with the virtual pair fastest, the ladder wants [(virtual pair)][Re | Im][(occupied pair)].  A CTA reads a 32 x 32 tile with
+// the virtual pair across the threads (16-byte elements), turns it in shared memory and writes with the occupied pair across
+// the threads: the planar X, the tile-major zero-padded X of the ladder kernels and tau.
 // X_ab[(e,F)][pl][(i,J)] = tab[i,J,e,F];  tau_ab = X + t1a[i,e] t1b[J,F]
-__global__ void k_build_Xab(Dims d, const double* __restrict__ t2p, const double* __restrict__ t1r,
-                            double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau)
+__global__ void __launch_bounds__(256) k_build_Xab(Dims d, const double* __restrict__ t2p, const double* __restrict__ t1r,
+                                                   double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau)
 {
-    const long long tot = (long long)d.v[0] * d.v[1] * d.oo;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
-        long long row = x / d.oo; int col = (int)(x - row * d.oo);
-        int e = (int)(row / d.v[1]), F = (int)(row - (long long)e * d.v[1]);
-        int i = col / d.o[1], J = col - i * d.o[1];
-        c128 z = ab_amp(t2p, d, i, J, e, F);
-        long long xa = (long long)i * d.v[0] + e, xb = d.n1a + (long long)J * d.v[1] + F;
-        double ar = t1r[xa], ai = t1r[d.n1 + xa], br = t1r[xb], bi = t1r[d.n1 + xb];
-        X[row * 2 * d.oo + col] = z.re;
-        X[row * 2 * d.oo + d.oo + col] = z.im;
-        Xt[xt_index(e, F, col, nFt, ncol, nt2)] = z.re;
-        Xt[xt_index(e, F, d.oo + col, nFt, ncol, nt2)] = z.im;
-        tau[row * 2 * d.oo + col] = z.re + ar * br - ai * bi;
-        tau[row * 2 * d.oo + d.oo + col] = z.im + ar * bi + ai * br;
+    __shared__ double sre[UP_T][UP_T + 1], sim[UP_T][UP_T + 1];
+    const int va = d.v[0], vb = d.v[1], ob = d.o[1];
+    const long long vv = (long long)va * vb, oo = d.oo, n1 = d.n1;
+    const int nCt = (int)((oo + UP_T - 1) / UP_T);
+    const long long nRt = (vv + UP_T - 1) / UP_T, nitem = nRt * nCt;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(t2p) + d.off_t2[2];
+    for (long long it = blockIdx.x; it < nitem; it += gridDim.x) {
+        const long long r0 = (it / nCt) * UP_T; const int c0 = (int)(it % nCt) * UP_T;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int col = c0 + ty + 8 * q; const long long row = r0 + tx;
+            double2 z = make_double2(0.0, 0.0);
+            if (col < oo && row < vv) z = src[(long long)col * vv + row];
+            sre[ty + 8 * q][tx] = z.x; sim[ty + 8 * q][tx] = z.y;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const long long row = r0 + ty + 8 * q; const int col = c0 + tx;
+            if (col < oo && row < vv) {
+                const double re = sre[tx][ty + 8 * q], im = sim[tx][ty + 8 * q];
+                const int e = (int)(row / vb), F = (int)(row - (long long)e * vb), i = col / ob, J = col - i * ob;
+                const long long xa = (long long)i * va + e, xb = d.n1a + (long long)J * vb + F;
+                const double ar = t1r[xa], ai = t1r[n1 + xa], br = t1r[xb], bi = t1r[n1 + xb];
+                X[row * 2 * oo + col] = re;
+                X[row * 2 * oo + oo + col] = im;
+                Xt[xt_index(e, F, col, nFt, ncol, nt2)] = re;
+                Xt[xt_index(e, F, (int)oo + col, nFt, ncol, nt2)] = im;
+                tau[row * 2 * oo + col] = re + ar * br - ai * bi;
+                tau[row * 2 * oo + oo + col] = im + ar * bi + ai * br;
+            }
+        }
     }
 }
 
-// X_ss[(e,f)][pl][(i<j)] = t_{ij}^{ef};  tau = X + t1[i,e] t1[j,f] - t1[i,f] t1[j,e]
-__global__ void k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const double* __restrict__ t1r,
-                            const int2* __restrict__ opairs, double* __restrict__ X, double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau, int anti)
+// X_ss[(e,f)][pl][(i<j)] = t_{ij}^{ef} = -X_ss[(f,e)];  tau = X + t1[i,e] t1[j,f] - t1[i,f] t1[j,e].  Rows e == f are zero: the
+// buffers are cleared at creation and those rows never written.  anti: rows e >= f of the tile-major X stay zero as well.
+__global__ void __launch_bounds__(256) k_build_Xss(Dims d, int s, const double* __restrict__ t2p, const double* __restrict__ t1r,
+                                                   const int2* __restrict__ opairs, const int2* __restrict__ vpairs, double* __restrict__ X,
+                                                   double* __restrict__ Xt, int nFt, int ncol, int nt2, double* __restrict__ tau, int anti)
 {
-    const int v = d.v[s], po = d.po[s];
-    const long long tot = (long long)v * v * po;
-    const long long o1 = s ? d.n1a : 0;
-    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < tot; x += (long long)gridDim.x * blockDim.x) {
-        long long row = x / po; int col = (int)(x - row * po);
-        int e = (int)(row / v), f = (int)(row - (long long)e * v);
-        int2 ij = opairs[col];
-        c128 z = ss_amp(t2p, d.off_t2[s], d.pv[s], ij.x, ij.y, e, f);
-        long long ie = o1 + (long long)ij.x * v + e, jf = o1 + (long long)ij.y * v + f;
-        long long iff = o1 + (long long)ij.x * v + f, je = o1 + (long long)ij.y * v + e;
-        double tr = t1r[ie] * t1r[jf] - t1r[d.n1 + ie] * t1r[d.n1 + jf] - (t1r[iff] * t1r[je] - t1r[d.n1 + iff] * t1r[d.n1 + je]);
-        double ti = t1r[ie] * t1r[d.n1 + jf] + t1r[d.n1 + ie] * t1r[jf] - (t1r[iff] * t1r[d.n1 + je] + t1r[d.n1 + iff] * t1r[je]);
-        X[row * 2 * po + col] = z.re;
-        X[row * 2 * po + po + col] = z.im;
-        if (!anti || e < f) {                 // antisymmetrised ladder: rows e >= f stay zero (cleared at creation)
-            Xt[xt_index(e, f, col, nFt, ncol, nt2)] = z.re;
-            Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = z.im;
+    __shared__ double sre[UP_T][UP_T + 1], sim[UP_T][UP_T + 1];
+    const int v = d.v[s], po = d.po[s], pv = d.pv[s];
+    const long long o1 = s ? d.n1a : 0, n1 = d.n1;
+    const int nCt = (po + UP_T - 1) / UP_T, nRt = (pv + UP_T - 1) / UP_T;
+    const long long nitem = (long long)nRt * nCt;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const double2* __restrict__ src = reinterpret_cast<const double2*>(t2p) + d.off_t2[s];
+    for (long long it = blockIdx.x; it < nitem; it += gridDim.x) {
+        const int r0 = (int)(it / nCt) * UP_T, c0 = (int)(it % nCt) * UP_T;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int col = c0 + ty + 8 * q, pr = r0 + tx;
+            double2 z = make_double2(0.0, 0.0);
+            if (col < po && pr < pv) z = src[(long long)col * pv + pr];
+            sre[ty + 8 * q][tx] = z.x; sim[ty + 8 * q][tx] = z.y;
         }
-        tau[row * 2 * po + col] = z.re + tr;
-        tau[row * 2 * po + po + col] = z.im + ti;
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int pr = r0 + ty + 8 * q, col = c0 + tx;
+            if (col < po && pr < pv) {
+                const double re = sre[tx][ty + 8 * q], im = sim[tx][ty + 8 * q];
+                const int2 ef = vpairs[pr], ij = opairs[col];
+                const int e = ef.x, f = ef.y;                       // e < f
+                const long long ie = o1 + (long long)ij.x * v + e, jf = o1 + (long long)ij.y * v + f;
+                const long long iff = o1 + (long long)ij.x * v + f, je = o1 + (long long)ij.y * v + e;
+                const double tr = t1r[ie] * t1r[jf] - t1r[n1 + ie] * t1r[n1 + jf] - (t1r[iff] * t1r[je] - t1r[n1 + iff] * t1r[n1 + je]);
+                const double ti = t1r[ie] * t1r[n1 + jf] + t1r[n1 + ie] * t1r[jf] - (t1r[iff] * t1r[n1 + je] + t1r[n1 + iff] * t1r[je]);
+                const long long ra = ((long long)e * v + f) * 2 * po, rb = ((long long)f * v + e) * 2 * po;
+                X[ra + col] = re; X[ra + po + col] = im;
+                X[rb + col] = -re; X[rb + po + col] = -im;
+                tau[ra + col] = re + tr; tau[ra + po + col] = im + ti;
+                tau[rb + col] = -re - tr; tau[rb + po + col] = -im - ti;
+                Xt[xt_index(e, f, col, nFt, ncol, nt2)] = re;
+                Xt[xt_index(e, f, po + col, nFt, ncol, nt2)] = im;
+                if (!anti) {
+                    Xt[xt_index(f, e, col, nFt, ncol, nt2)] = -re;
+                    Xt[xt_index(f, e, po + col, nFt, ncol, nt2)] = -im;
+                }
+            }
+        }
     }
 }
 

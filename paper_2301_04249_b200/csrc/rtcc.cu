@@ -237,10 +237,24 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
             }
         }
     }
-    EW(c, k_build_Xab, (long long)d.v[0] * d.v[1] * d.oo, d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8, (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
+    {
+        const long long nab = (((long long)d.v[0] * d.v[1] + UP_T - 1) / UP_T) * ((d.oo + UP_T - 1) / UP_T);
+        if (d.oo > 0) {
+            k_build_Xab<<<(int)std::min<long long>(nab, (long long)c->num_sms * 16), 256, 0, ST>>>(d, t2p, c->t1r, c->Xab, c->Xt_ab, (d.v[1] + 7) / 8,
+                                                                                       (2 * d.oo + c->nt2_ab - 1) / c->nt2_ab, c->nt2_ab, c->tauab);
+            c->launches++;
+        }
+    }
     for (int s = 0; s < 2; ++s)
         if (d.po[s] > 0)
-            EW(c, k_build_Xss, (long long)d.v[s] * d.v[s] * d.po[s], d, s, t2p, c->t1r, c->opairs[s], c->Xss[s], c->Xt_ss[s], (d.v[s] + 7) / 8, (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->tauss[s], c->anti_ss[s]);
+        {
+            const long long nss = (long long)((d.pv[s] + UP_T - 1) / UP_T) * ((d.po[s] + UP_T - 1) / UP_T);
+            if (nss > 0) {
+                k_build_Xss<<<(int)std::min<long long>(nss, (long long)c->num_sms * 16), 256, 0, ST>>>(d, s, t2p, c->t1r, c->opairs[s], c->vpairs[s], c->Xss[s],
+                    c->Xt_ss[s], (d.v[s] + 7) / 8, (2 * d.po[s] + c->nt2_ss[s] - 1) / c->nt2_ss[s], c->nt2_ss[s], c->tauss[s], c->anti_ss[s]);
+                c->launches++;
+            }
+        }
 
     if (par) CK(cudaEventRecord(c->evs[0], c->S[0]));     // evs[0]: unpacked layouts ready
 
@@ -1615,7 +1629,10 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
             DA(c->Ft[s], 2 * nn, s ? "Ft1" : "Ft0");
             DA(c->Kx[s], (long long)d.o[s] * d.v[s] * d.o[s] * d.v[s], s ? "Kx1" : "Kx0");
             const int po = d.po[s], v = d.v[s], o = d.o[s];
-            if (!c->lean) DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
+            if (!c->lean) {
+                DA(c->Xss[s], (long long)v * v * 2 * po, s ? "Xss1" : "Xss0");
+                CKC(cudaMemsetAsync(c->Xss[s], 0, (size_t)std::max<long long>((long long)v * v * 2 * po, 1) * 8, c->st));   // rows e == f stay zero
+            }
             {
                 const int nt2 = 2 * po <= 64 ? 64 : 128;
                 c->nt2_ss[s] = nt2;
@@ -1641,6 +1658,7 @@ int rtcc_create(rtcc_ctx** out, int oa, int ob, int va, int vb, int NQ, const do
                 DA(c->cmp[s], d.pv[s], nullptr);
             } else {
                 DA(c->tauss[s], (long long)v * v * 2 * po, nullptr);
+                CKC(cudaMemsetAsync(c->tauss[s], 0, (size_t)std::max<long long>((long long)v * v * 2 * po, 1) * 8, c->st));
                 DA(c->Yss[s], nn * 2 * po, s ? "Yss1" : "Yss0");
                 DA(c->Zv[s], (long long)v * v * 2 * po, s ? "Zv1" : "Zv0");
                 CKC(cudaMemsetAsync(c->Yss[s], 0, (size_t)(nn * 2 * po > 0 ? nn * 2 * po : 1) * 8, c->st));
