@@ -113,12 +113,17 @@ __global__ void __launch_bounds__(256) k_unpack_ab(Dims d, const double* __restr
         const int M = (int)(k % ob), i = (int)(k / ob);
         const long long base = ((long long)i * ob + M) * va;
         __syncthreads();
+        double2 zz[UP_T / 8];                           // all loads of the tile first: they are in flight together
 #pragma unroll
         for (int q = 0; q < UP_T / 8; ++q) {
             const int a = a0 + ty + 8 * q, E = E0 + tx;
-            double2 z = make_double2(0.0, 0.0);
+            zz[q] = (a < va && E < vb) ? src[(base + a) * vb + E] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int a = a0 + ty + 8 * q, E = E0 + tx;
+            const double2 z = zz[q];
             if (a < va && E < vb) {
-                z = src[(base + a) * vb + E];
                 const long long r = (long long)i * va + a, c = d.n1a + (long long)M * vb + E;
                 Tsc[r * ld + c] = z.x;
                 Tsc[r * ld + n1 + c] = z.y;
@@ -163,12 +168,17 @@ __global__ void __launch_bounds__(256) k_unpack_ss(Dims d, int s, const int2* __
         const int2 im_ = opairs[pim];
         const long long ri = off + (long long)im_.x * v, rm = off + (long long)im_.y * v;    // first row / column of (i,.) and (m,.)
         __syncthreads();
+        double2 zz[UP_T / 8];
 #pragma unroll
         for (int q = 0; q < UP_T / 8; ++q) {
             const int e = e0 + ty + 8 * q, a = a0 + tx;
-            double2 z = make_double2(0.0, 0.0);
+            zz[q] = (a < e && e < v) ? src[(long long)pim * pv + pair_index(a, e)] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int q = 0; q < UP_T / 8; ++q) {
+            const int e = e0 + ty + 8 * q, a = a0 + tx;
+            const double2 z = zz[q];
             if (a < e && e < v) {
-                z = src[(long long)pim * pv + pair_index(a, e)];
                 // destinations whose fastest index is a:  T[(i,e),(m,a)] = -t,  T[(m,e),(i,a)] = +t
                 long long r = ri + e, c = rm + a;
                 Tsc[r * ld + c] = -z.x; Tsc[r * ld + n1 + c] = -z.y;
