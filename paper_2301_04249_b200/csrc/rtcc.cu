@@ -478,6 +478,7 @@ int residual_pipeline(rtcc_ctx* c, const double* x, double* r)
         setC(g, 0, ld1, 0, 1);
         ops_cc(g, c->Nq, n1, c->Nq, n1, c->Zsc, n1);
         g.alpha = 0.5;
+        g.sym_upper = 1;                  // N^T N is symmetric and the assembly only uses Z + Z^T: half of the tiles
         run(c, g);
     }
 

@@ -40,6 +40,8 @@ struct TcGemm {
     int ksplit;                              // deterministic split-K (partials in ws, reduced by a 2nd kernel)
     double* ws;
     const long long* cm_table;               // optional: offset of output row m (replaces the two-level row index of C)
+    int sym_upper;                           // the product is symmetric and only C + C^T is used downstream: tiles above the diagonal
+                                             // are computed and doubled, diagonal tiles computed, tiles below written as alpha*0 + beta*C
 };
 
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc, bool valid)
@@ -135,7 +137,9 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
     const int per = (nkt + g.ksplit - 1) / g.ksplit;
     const int kt0 = split * per;
     const int kt1 = min(nkt, kt0 + per);
-    const int nk = max(kt1 - kt0, 0);
+    const bool lower = g.sym_upper && m0 > n0;
+    const double symfac = (g.sym_upper && m0 < n0) ? 2.0 : 1.0;
+    const int nk = lower ? 0 : max(kt1 - kt0, 0);
     const int nph = g.nphase[db];
     const int total = nk * nph;
 
@@ -282,15 +286,15 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 48) tcgemm_kernel(cons
 #pragma unroll
             for (int j = 0; j < TN; ++j) {
                 int n = n0 + wn0 + 8 * j + 2 * lc;
-                if (n < g.N) W[(long long)m * g.N + n] = sgn * acc[i][j][0];
-                if (n + 1 < g.N) W[(long long)m * g.N + n + 1] = sgn * acc[i][j][1];
+                if (n < g.N) W[(long long)m * g.N + n] = sgn * symfac * acc[i][j][0];
+                if (n + 1 < g.N) W[(long long)m * g.N + n + 1] = sgn * symfac * acc[i][j][1];
             }
         }
         return;
     }
     double* C = g.C[db] + sb * g.sbC;
     double* C2 = g.C2[db] ? g.C2[db] + sb * g.sbC : nullptr;
-    const double al = g.alpha * sgn, be = g.beta;
+    const double al = g.alpha * sgn * symfac, be = g.beta;
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
         int m = m0 + wm0 + 8 * i + lr;
@@ -379,7 +383,8 @@ inline int tcgemm_launch(TcGemm g, cudaStream_t st, long long ws_cap, int num_sm
     if (flops_out) {
         int tot_ph = 0;
         for (int b = 0; b < g.nb; ++b) tot_ph += g.nphase[b];
-        *flops_out += 2.0 * g.M * g.N * (double)g.K * tot_ph * g.nsb;
+        const double nt = (double)((g.M + BM - 1) / BM);
+        *flops_out += 2.0 * g.M * g.N * (double)g.K * tot_ph * g.nsb * (g.sym_upper ? 0.5 * (nt + 1.0) / nt : 1.0);
     }
     dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, nbt * ks);
     if (big) {
